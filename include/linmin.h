@@ -1,0 +1,142 @@
+/*
+ * linmin.h -- C ABI of liblinmin.so: per-pixel fully constrained linear unmixing on one B200.
+ *
+ * The operation (citations: /root/reference/PAPER.md line + section/equation):
+ *   PAPER.md:48-50 (sec. 2.1, eq. 1)   X = A.S + E, zero-mean Gaussian noise.
+ *   PAPER.md:54    (eq. 2)             F = sum_pixels sum_channels (X - A.S)^2, separable per pixel.
+ *   PAPER.md:63    (eq. 3)             every mixing coefficient >= 0.
+ *   PAPER.md:68    (eq. 4)             the coefficients of a pixel sum to one.
+ *   PAPER.md:71-73 (sec. 2.2)          solved by IPLS, a primal-dual interior-point least-squares
+ *                                      method; convexity of F suffices for convergence.
+ *   PAPER.md:88    (sec. 2.3)          "an estimation of the error on the mixing coefficient is
+ *                                      directly provided by the Hessian".
+ *   PAPER.md:143, 246, 252             the fit RMS, compared with the noise level.
+ *
+ * Notation here follows BASELINE.json (the paper writes the transpose): for each of N pixels, a
+ * spectrum y (L channels) is fitted by a = argmin ||y - A a||^2 s.t. a >= 0, sum(a) = 1 against ONE
+ * shared library A (L x R; column r is endmember r; the paper's S^T).  Outputs per pixel: the
+ * minimiser a (R), its first-order standard deviations given the per-channel noise std sigma
+ * (reading R3), and the RMS residual sqrt(mean_l (y - A a)_l^2) (reading R8).
+ *
+ * Layouts (all float32, C order):
+ *   A[l*R + r]                       L x R, row-major (channel-major)
+ *   Y[p*ldY + l]                     one spectrum = L contiguous floats; ldY >= L elements
+ *   sigma                            NULL            -> sigma == 1 (noise amplification factors)
+ *                                    stride 0        -> one shared vector sigma[l], l < L
+ *                                    stride s >= L   -> per pixel, sigma[p*s + l]
+ *   coeffs_out[p*R + r], coeff_sigma_out[p*R + r], resid_out[p]
+ *
+ * Ownership: every pointer is owned by the caller; the library never frees or reallocates caller
+ * memory.  Outputs must not alias inputs or each other.  `coeff_sigma_out`, `resid_out`, `sigma`
+ * and `opts` may be NULL (output skipped / defaults).  Internal workspace (O(R^2 + L R) bytes) is
+ * owned by the linmin_library handle.
+ *
+ * Device entry points (linmin_unmix, linmin_unmix_lib): every data pointer is a DEVICE pointer on
+ * the current CUDA device.  Work is enqueued on opts->stream and the call returns without waiting
+ * for it; there is no host round-trip inside the per-pixel iteration.  Argument errors are returned
+ * synchronously; asynchronous CUDA errors surface at the next call or stream synchronisation.
+ * Host entry point (linmin_unmix_host): every data pointer is a HOST pointer (pinned memory gives
+ * full copy bandwidth); the call stages chunks through the device and returns when outputs are
+ * complete.
+ *
+ * There is no CPU fallback anywhere: without a CUDA device every compute call fails with
+ * LINMIN_ERR_CUDA.  No exceptions cross this ABI; no global mutable state; calls on distinct
+ * streams / handles are thread-safe.
+ */
+#ifndef LINMIN_H_
+#define LINMIN_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LINMIN_VERSION 100 /* 0.1.0 */
+
+/* status codes: 0 ok, < 0 error, > 0 warning (results valid) */
+#define LINMIN_OK 0
+#define LINMIN_ERR_INVALID_ARGUMENT (-1)  /* NULL required pointer, N < 0, L < 1, R < 1, ldY < L, bad stride, struct_size */
+#define LINMIN_ERR_UNSUPPORTED_SIZE (-2)  /* R > LINMIN_MAX_R or L > LINMIN_MAX_L */
+#define LINMIN_ERR_NOT_IMPLEMENTED (-3)   /* a constraint / weighting option that is not built yet */
+#define LINMIN_ERR_CUDA (-4)              /* CUDA runtime failure (including: no device) */
+#define LINMIN_ERR_OUT_OF_MEMORY (-5)
+#define LINMIN_ERR_LIBRARY_NONFINITE (-6) /* A contains NaN or Inf */
+#define LINMIN_WARN_RANK_DEFICIENT 1      /* R > L: minimiser may be non-unique (PAPER.md:92 asks R <= L) */
+
+#define LINMIN_MAX_R 256
+#define LINMIN_MAX_L 512
+
+/* constraint (sto / slo / pos options of IPLS) */
+#define LINMIN_CONSTRAINT_SUM_TO_ONE 0        /* eq. 3 + eq. 4: the hot path */
+#define LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE 1 /* not implemented yet */
+#define LINMIN_CONSTRAINT_POSITIVITY_ONLY 2    /* not implemented yet */
+
+/* weighting (eq. 5-6) */
+#define LINMIN_WEIGHTING_NONE 0               /* unweighted fit; sigma used for propagation only */
+#define LINMIN_WEIGHTING_SHARED_COVARIANCE 1  /* not implemented yet */
+
+/* per-pixel info word (opts->info_out): flags in bits 0-7, then three counters */
+#define LINMIN_INFO_CONVERGED 0x01      /* IPLS met its stopping rule */
+#define LINMIN_INFO_MAX_ITER 0x02       /* IPLS stopped at max_iter (the exact finish still ran) */
+#define LINMIN_INFO_NONFINITE_INPUT 0x04 /* y has NaN/Inf: all outputs of the pixel are NaN */
+#define LINMIN_INFO_CHOL_REGULARISED 0x08 /* a Newton-matrix pivot was clamped */
+#define LINMIN_INFO_FINISH_FALLBACK 0x10 /* finish hit its pivot/support cap: result feasible, near-optimal, not certified */
+#define LINMIN_INFO_BAD_SIGMA 0x20      /* sigma <= 0 or non-finite: coeff_sigma of the pixel is NaN */
+#define LINMIN_INFO_ITERATIONS(w) (((w) >> 8) & 0xff)  /* IPLS Newton iterations */
+#define LINMIN_INFO_PIVOTS(w) (((w) >> 16) & 0xff)     /* finish support changes */
+#define LINMIN_INFO_SUPPORT(w) (((w) >> 24) & 0xff)    /* number of non-zero coefficients */
+
+typedef struct linmin_opts {
+    uint32_t struct_size;       /* sizeof(linmin_opts); anything else -> LINMIN_ERR_INVALID_ARGUMENT */
+    void *stream;               /* cudaStream_t; NULL = default stream */
+    int64_t ldY;                /* elements between consecutive spectra in Y; 0 -> L */
+    int64_t sigma_pixel_stride; /* 0 -> shared sigma[L]; else elements between pixels (>= L) */
+    int32_t constraint;         /* LINMIN_CONSTRAINT_* */
+    int32_t weighting;          /* LINMIN_WEIGHTING_* */
+    int32_t max_iter;           /* IPLS iteration cap, 1..255; 0 -> 50 */
+    float gap_tol;              /* stop when a'lambda <= gap_tol * scale; 0 -> 1e-8 */
+    float feas_tol;             /* ... and dual/primal residuals <= feas_tol (* scale); 0 -> 1e-6 */
+    int32_t *info_out;          /* optional int32[N] (device pointer; host pointer for linmin_unmix_host) */
+    int32_t deterministic;      /* results never depend on tiling or scheduling; kept for ABI, always on */
+    int32_t reserved;
+} linmin_opts;
+
+typedef struct linmin_library linmin_library; /* opaque: precomputed per-library data on the device */
+
+/* Once-per-library precompute ("S.S^T"): centred library, Gram
+ * matrices in fp32 and fp64.  A is a DEVICE pointer (copied; the caller may free it afterwards).
+ * Synchronises the stream once to validate A.  Returns LINMIN_OK, LINMIN_WARN_RANK_DEFICIENT
+ * (handle valid) or an error (*lib = NULL).  Only opts->stream is read. */
+int linmin_library_create(const float *A, int32_t L, int32_t R, const linmin_opts *opts,
+                          linmin_library **lib);
+
+/* Frees the handle's device memory (stream-ordered after all work enqueued with it). NULL is a no-op. */
+void linmin_library_destroy(linmin_library *lib);
+
+/* Unmix N spectra against a precomputed library.  Device pointers.  N == 0 is a no-op. */
+int linmin_unmix_lib(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
+                     const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out,
+                     float *resid_out);
+
+/* One-shot form: linmin_library_create + linmin_unmix_lib + linmin_library_destroy. Device pointers. */
+int linmin_unmix(const float *A, const float *Y, const float *sigma, int64_t N, int32_t L, int32_t R,
+                 const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out, float *resid_out);
+
+/* Same operation with HOST buffers (A, Y, sigma, outputs, opts->info_out): chunks of pixels are
+ * copied host->device, solved and copied back on alternating streams so that copies overlap the
+ * kernels.  Blocks until the outputs are complete.  opts->stream is ignored. */
+int linmin_unmix_host(const float *A, const float *Y, const float *sigma, int64_t N, int32_t L,
+                      int32_t R, const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out,
+                      float *resid_out);
+
+/* Number of kernel launches the last linmin_unmix_lib call on this handle enqueued (for reports). */
+int linmin_library_last_launches(const linmin_library *lib);
+
+const char *linmin_strerror(int code);
+int linmin_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LINMIN_H_ */

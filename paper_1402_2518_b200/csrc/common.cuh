@@ -1,0 +1,61 @@
+// common.cuh -- shared declarations of the LinMin CUDA path (sm_100a).
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/linmin.h"
+
+namespace linmin {
+
+// Device-side view of the once-per-library precompute.
+struct LibView {
+    int L, R;
+    const float *A;     // L x R, caller's library (copied into the handle)
+    const float *Ac;    // L x R, centred: Ac[l][r] = A[l][r] - c[l], c[l] = mean_r A[l][r]
+    const float *c;     // L
+    const float *Gc;    // R x R fp32, Gc = Ac' Ac accumulated in fp64 (drives IPLS)
+    const double *G64;  // R x R fp64, G = A' A (uncentred, exact data; drives the finish)
+    float gdmax;        // max_i Gc[i][i]
+};
+
+struct SolveParams {
+    const float *Y;
+    const float *sigma;
+    int64_t N;
+    int64_t ldY;
+    int64_t sigma_stride;   // 0 shared, else per pixel
+    int has_sigma;
+    int max_iter;
+    float gap_tol, feas_tol;
+    float *coeffs;          // N x R (IPLS iterate in, final coefficients out)
+    float *coeff_sigma;     // N x R or NULL
+    float *resid;           // N or NULL
+    int32_t *info;          // N or NULL
+};
+
+// column-major packed lower triangle of an n x n matrix: (i, j), i >= j
+__host__ __device__ __forceinline__ int cm(int n, int i, int j) { return j * n - (j * (j - 1)) / 2 + (i - j); }
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ float warp_min(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+}  // namespace linmin

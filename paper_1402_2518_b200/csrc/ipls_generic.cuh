@@ -1,0 +1,286 @@
+// ipls_generic.cuh -- projection + IPLS (primal-dual interior-point least squares), any R <= 256.
+//
+// PAPER.md:71-73 (sec. 2.2) names IPLS (Chouzenoux et al.) and states only that convexity of F
+// gives convergence; it prints no steps (reading R1).  The iteration below is a standard
+// Mehrotra predictor-corrector primal-dual method on the per-pixel QP
+//      min 1/2 a'G a - b'a   s.t.  a >= 0 (multipliers lambda),  1'a = 1 (multiplier nu)
+// with G = Ac'Ac, b = Ac'(y - c) (centred library, precompute.cuh).  Perturbed KKT system:
+//      G a - b - lambda + nu 1 = 0,   1'a = 1,   a_i lambda_i = mu.
+// One Newton step:  M = G + diag(lambda/a);  v = M^-1 1;  u = M^-1( -(G a - b + nu 1) + c/a );
+//      dnu = (1'u + r_p)/(1'v);  da = u - v dnu;  dlambda = -lambda + c/a - (lambda/a) da;
+// c = 0 (predictor), then c = sigma mu 1 - da_aff * dlambda_aff with sigma = (mu_aff/mu)^3
+// (corrector); fraction-to-boundary 0.995, separate primal and dual step lengths.
+//
+// This generic kernel keeps everything of a pixel in shared memory and lets a TEAM of threads
+// (a warp, or the whole CTA for R > 64) cooperate on the Cholesky factorisation and the triangular
+// solves.  It is the any-size reference path; R = 32 has a register-blocked kernel of its own.
+#pragma once
+#include "common.cuh"
+
+namespace linmin {
+
+template <int TEAM>
+struct TeamOps;
+
+template <>
+struct TeamOps<32> {
+    static __device__ __forceinline__ int tid() { return threadIdx.x & 31; }
+    static __device__ __forceinline__ void sync() { __syncwarp(); }
+    static __device__ __forceinline__ float sum(float v, float *) { return warp_sum(v); }
+    static __device__ __forceinline__ float max(float v, float *) { return warp_max(v); }
+    static __device__ __forceinline__ float min(float v, float *) { return warp_min(v); }
+};
+
+// the whole CTA is one team; `red` is a 2 x 32-float scratch area in shared memory
+template <int TEAM>
+struct TeamOps {
+    static __device__ __forceinline__ int tid() { return threadIdx.x; }
+    static __device__ __forceinline__ void sync() { __syncthreads(); }
+    template <typename Op>
+    static __device__ __forceinline__ float reduce(float v, float *red, Op op, float ident) {
+        int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v = op(v, __shfl_xor_sync(0xffffffffu, v, o));
+        if (lane == 0) red[w] = v;
+        __syncthreads();
+        float r = (lane < TEAM / 32) ? red[lane] : ident;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) r = op(r, __shfl_xor_sync(0xffffffffu, r, o));
+        __syncthreads();
+        return r;
+    }
+    static __device__ __forceinline__ float sum(float v, float *red) {
+        return reduce(v, red, [](float a, float b) { return a + b; }, 0.0f);
+    }
+    static __device__ __forceinline__ float max(float v, float *red) {
+        return reduce(v, red, [](float a, float b) { return fmaxf(a, b); }, -INFINITY);
+    }
+    static __device__ __forceinline__ float min(float v, float *red) {
+        return reduce(v, red, [](float a, float b) { return fminf(a, b); }, INFINITY);
+    }
+};
+
+// In-place left-looking Cholesky of the packed (column-major lower) n x n matrix Mp.
+// dinv[j] = 1/L_jj; the diagonal of Mp keeps the ORIGINAL M_jj (every thread re-derives the pivot
+// from it, so it must not be overwritten while the column is in flight; L_jj = 1/dinv[j]).
+// A pivot below `floorv` is clamped (returns true if that happened).
+template <int TEAM, typename T>
+__device__ __forceinline__ bool team_cholesky(T *Mp, T *dinv, int n, T floorv) {
+    using Ops = TeamOps<TEAM>;
+    const int t = Ops::tid();
+    bool clamped = false;
+    for (int j = 0; j < n; ++j) {
+        T sj = Mp[cm(n, j, j)];
+        for (int k = 0; k < j; ++k) {
+            T ljk = Mp[cm(n, j, k)];
+            sj -= ljk * ljk;
+        }
+        if (!(sj > floorv)) { sj = floorv; clamped = true; }
+        T dj = (T)1 / sqrt(sj);
+        for (int i = j + t; i < n; i += TEAM) {
+            if (i == j) {
+                dinv[j] = dj;
+            } else {
+                T s = Mp[cm(n, i, j)];
+                for (int k = 0; k < j; ++k) s -= Mp[cm(n, i, k)] * Mp[cm(n, j, k)];
+                Mp[cm(n, i, j)] = s * dj;
+            }
+        }
+        Ops::sync();
+    }
+    return clamped;
+}
+
+// Solve (L L') x = rhs in place for NRHS right-hand sides stored at x[0], x[1] (each n long).
+template <int TEAM, int NRHS, typename T>
+__device__ __forceinline__ void team_solve(const T *Mp, const T *dinv, int n, T *x0, T *x1) {
+    using Ops = TeamOps<TEAM>;
+    const int t = Ops::tid();
+    for (int j = 0; j < n; ++j) {          // forward: L z = rhs
+        T z0 = x0[j] * dinv[j];
+        T z1 = NRHS > 1 ? x1[j] * dinv[j] : (T)0;
+        for (int i = j + 1 + t; i < n; i += TEAM) {
+            T l = Mp[cm(n, i, j)];
+            x0[i] -= l * z0;
+            if (NRHS > 1) x1[i] -= l * z1;
+        }
+        Ops::sync();
+    }
+    for (int i = t; i < n; i += TEAM) {
+        x0[i] *= dinv[i];
+        if (NRHS > 1) x1[i] *= dinv[i];
+    }
+    Ops::sync();
+    for (int j = n - 1; j >= 0; --j) {     // backward: L' x = z
+        T z0 = x0[j] * dinv[j];
+        T z1 = NRHS > 1 ? x1[j] * dinv[j] : (T)0;
+        for (int i = t; i < j; i += TEAM) {
+            T l = Mp[cm(n, j, i)];
+            x0[i] -= l * z0;
+            if (NRHS > 1) x1[i] -= l * z1;
+        }
+        Ops::sync();
+    }
+    for (int i = t; i < n; i += TEAM) {
+        x0[i] *= dinv[i];
+        if (NRHS > 1) x1[i] *= dinv[i];
+    }
+    Ops::sync();
+}
+
+__host__ __device__ inline size_t ipls_generic_team_floats(int L, int R) {
+    return (size_t)9 * R + L + (size_t)R * (R + 1) / 2 + 64;
+}
+
+// grid-stride over pixels; TEAM == 32: one warp per pixel, blockDim.x/32 pixels per CTA pass;
+// TEAM == blockDim.x: one pixel per CTA pass.
+template <int TEAM>
+__global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolveParams prm) {
+    using Ops = TeamOps<TEAM>;
+    extern __shared__ __align__(16) float smem[];
+    const int L = lib.L, R = lib.R;
+    const int teams_per_cta = blockDim.x / TEAM;
+    const int team = threadIdx.x / TEAM;
+    const int t = Ops::tid();
+    float *base = smem + (size_t)team * ipls_generic_team_floats(L, R);
+    float *a = base, *lam = a + R, *b = lam + R, *w = b + R, *u = w + R, *v = u + R, *da = v + R,
+          *dl = da + R, *dinv = dl + R, *yc = dinv + R, *red = yc + L, *Mp = red + 64;
+    const float fR = (float)R;
+    const float tau = 0.995f;
+
+    for (int64_t p = (int64_t)blockIdx.x * teams_per_cta + team; p < prm.N;
+         p += (int64_t)gridDim.x * teams_per_cta) {
+        // ---- load spectrum, centre it, detect non-finite input
+        const float *y = prm.Y + p * prm.ldY;
+        float badf = 0.0f;
+        for (int l = t; l < L; l += TEAM) {
+            float yv = y[l];
+            if (!isfinite(yv)) badf = 1.0f;
+            yc[l] = yv - lib.c[l];
+        }
+        Ops::sync();
+        badf = Ops::max(badf, red);
+        if (badf > 0.0f) {
+            for (int i = t; i < R; i += TEAM) prm.coeffs[p * R + i] = 1.0f / fR;
+            if (prm.info && t == 0) prm.info[p] = LINMIN_INFO_NONFINITE_INPUT;
+            Ops::sync();
+            continue;
+        }
+        // ---- projection b = Ac'(y - c)   ("X.S^T")
+        float bmax = 0.0f;
+        for (int i = t; i < R; i += TEAM) {
+            float s = 0.0f;
+            for (int l = 0; l < L; ++l) s = fmaf(lib.Ac[(size_t)l * R + i], yc[l], s);
+            b[i] = s;
+            bmax = fmaxf(bmax, fabsf(s));
+            a[i] = 1.0f / fR;
+        }
+        bmax = Ops::max(bmax, red);
+        const float sc = fmaxf(bmax, 1e-3f * lib.gdmax);
+        // start: a = 1/R, nu = 0, lambda = max(||G a - b||_inf, 1e-3 gdmax)
+        float g0 = 0.0f;
+        Ops::sync();
+        for (int i = t; i < R; i += TEAM) {
+            float s = 0.0f;
+            for (int j = 0; j < R; ++j) s = fmaf(lib.Gc[(size_t)j * R + i], a[j], s);
+            g0 = fmaxf(g0, fabsf(s - b[i]));
+        }
+        g0 = Ops::max(g0, red);
+        const float lam0 = fmaxf(g0, 1e-3f * lib.gdmax);
+        for (int i = t; i < R; i += TEAM) lam[i] = lam0;
+        float nu = 0.0f;
+        int iters = 0, flags = 0;
+        Ops::sync();
+
+        for (int it = 0;; ++it) {
+            // ---- residuals
+            float rdmax = 0.0f, suma = 0.0f, gap = 0.0f;
+            for (int i = t; i < R; i += TEAM) {
+                float s = 0.0f;
+                for (int j = 0; j < R; ++j) s = fmaf(lib.Gc[(size_t)j * R + i], a[j], s);
+                float wi = s - b[i] + nu;
+                w[i] = wi;
+                rdmax = fmaxf(rdmax, fabsf(wi - lam[i]));
+                suma += a[i];
+                gap = fmaf(a[i], lam[i], gap);
+            }
+            rdmax = Ops::max(rdmax, red);
+            suma = Ops::sum(suma, red);
+            gap = Ops::sum(gap, red);
+            const float rp = suma - 1.0f;
+            if (gap <= prm.gap_tol * sc && rdmax <= prm.feas_tol * sc && fabsf(rp) <= prm.feas_tol) {
+                flags |= LINMIN_INFO_CONVERGED;
+                break;
+            }
+            if (it >= prm.max_iter) { flags |= LINMIN_INFO_MAX_ITER; break; }
+            ++iters;
+            const float mu = gap / fR;
+            // ---- Newton matrix M = Gc + diag(lambda / a), packed lower, then Cholesky
+            for (int j = 0; j < R; ++j)
+                for (int i = j + t; i < R; i += TEAM) {
+                    float m = lib.Gc[(size_t)j * R + i];
+                    if (i == j) m += lam[i] / a[i];
+                    Mp[cm(R, i, j)] = m;
+                }
+            Ops::sync();
+            if (team_cholesky<TEAM, float>(Mp, dinv, R, 1e-12f * lib.gdmax)) flags |= LINMIN_INFO_CHOL_REGULARISED;
+            // ---- predictor
+            for (int i = t; i < R; i += TEAM) { u[i] = -w[i]; v[i] = 1.0f; }
+            Ops::sync();
+            team_solve<TEAM, 2, float>(Mp, dinv, R, u, v);
+            float su = 0.0f, sv = 0.0f;
+            for (int i = t; i < R; i += TEAM) { su += u[i]; sv += v[i]; }
+            su = Ops::sum(su, red);
+            sv = Ops::sum(sv, red);
+            float dnu = (su + rp) / sv;
+            float ap = INFINITY, ad = INFINITY;
+            for (int i = t; i < R; i += TEAM) {
+                float dai = u[i] - v[i] * dnu;
+                float dli = -lam[i] - (lam[i] / a[i]) * dai;
+                da[i] = dai; dl[i] = dli;
+                if (dai < 0.0f) ap = fminf(ap, -a[i] / dai);
+                if (dli < 0.0f) ad = fminf(ad, -lam[i] / dli);
+            }
+            ap = fminf(1.0f, Ops::min(ap, red));
+            ad = fminf(1.0f, Ops::min(ad, red));
+            float mua = 0.0f;
+            for (int i = t; i < R; i += TEAM) mua = fmaf(a[i] + ap * da[i], lam[i] + ad * dl[i], mua);
+            mua = Ops::sum(mua, red) / fR;
+            float sg = mua / mu;
+            sg = fminf(1.0f, fmaxf(0.0f, sg * sg * sg));
+            // ---- corrector
+            for (int i = t; i < R; i += TEAM) {
+                float cc = sg * mu - da[i] * dl[i];
+                dl[i] = cc;
+                u[i] = -w[i] + cc / a[i];
+            }
+            Ops::sync();
+            team_solve<TEAM, 1, float>(Mp, dinv, R, u, nullptr);
+            su = 0.0f;
+            for (int i = t; i < R; i += TEAM) su += u[i];
+            su = Ops::sum(su, red);
+            dnu = (su + rp) / sv;
+            ap = INFINITY; ad = INFINITY;
+            for (int i = t; i < R; i += TEAM) {
+                float dai = u[i] - v[i] * dnu;
+                float dli = -lam[i] + dl[i] / a[i] - (lam[i] / a[i]) * dai;
+                da[i] = dai; dl[i] = dli;
+                if (dai < 0.0f) ap = fminf(ap, -a[i] / dai);
+                if (dli < 0.0f) ad = fminf(ad, -lam[i] / dli);
+            }
+            ap = fminf(1.0f, tau * Ops::min(ap, red));
+            ad = fminf(1.0f, tau * Ops::min(ad, red));
+            for (int i = t; i < R; i += TEAM) {
+                a[i] = fmaxf(fmaf(ap, da[i], a[i]), 1e-18f);
+                lam[i] = fmaxf(fmaf(ad, dl[i], lam[i]), 1e-18f * lam0);
+            }
+            nu = fmaf(ad, dnu, nu);
+            Ops::sync();
+        }
+        for (int i = t; i < R; i += TEAM) prm.coeffs[p * R + i] = a[i];
+        if (prm.info && t == 0) prm.info[p] = flags | (iters << 8);
+        Ops::sync();
+    }
+}
+
+}  // namespace linmin

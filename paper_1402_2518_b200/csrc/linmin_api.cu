@@ -1,0 +1,375 @@
+// linmin_api.cu -- C ABI of liblinmin.so (see include/linmin.h for the contract).
+// Host logic only: argument validation, the library handle, kernel launches, the host-buffer pipeline.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "finish.cuh"
+#include "ipls_generic.cuh"
+#include "ipls_r32.cuh"
+#include "precompute.cuh"
+
+using namespace linmin;
+
+struct linmin_library {
+    int L = 0, R = 0;
+    int device = 0;
+    int sm_count = 0;
+    cudaStream_t stream = nullptr;   // stream the handle was created on (frees are ordered on it)
+    float *A = nullptr, *Ac = nullptr, *c = nullptr, *Gc = nullptr;
+    double *G64 = nullptr;
+    float gdmax = 0.0f;
+    mutable int last_launches = 0;
+};
+
+namespace {
+
+int cuda_status(cudaError_t e) {
+    if (e == cudaSuccess) return LINMIN_OK;
+    if (e == cudaErrorMemoryAllocation) return LINMIN_ERR_OUT_OF_MEMORY;
+    return LINMIN_ERR_CUDA;
+}
+
+#define CK(call)                                   \
+    do {                                           \
+        cudaError_t e__ = (call);                  \
+        if (e__ != cudaSuccess) {                  \
+            (void)cudaGetLastError();              \
+            return cuda_status(e__);               \
+        }                                          \
+    } while (0)
+
+struct Resolved {
+    cudaStream_t stream;
+    int64_t ldY, sstride;
+    int max_iter;
+    float gap_tol, feas_tol;
+    int32_t *info;
+};
+
+int resolve_opts(const linmin_opts *o, int L, Resolved *r) {
+    r->stream = nullptr; r->ldY = L; r->sstride = 0; r->max_iter = 50;
+    r->gap_tol = 1e-8f; r->feas_tol = 1e-6f; r->info = nullptr;
+    if (!o) return LINMIN_OK;
+    if (o->struct_size != sizeof(linmin_opts)) return LINMIN_ERR_INVALID_ARGUMENT;
+    if (o->constraint != LINMIN_CONSTRAINT_SUM_TO_ONE) {
+        if (o->constraint == LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE || o->constraint == LINMIN_CONSTRAINT_POSITIVITY_ONLY)
+            return LINMIN_ERR_NOT_IMPLEMENTED;
+        return LINMIN_ERR_INVALID_ARGUMENT;
+    }
+    if (o->weighting != LINMIN_WEIGHTING_NONE) {
+        if (o->weighting == LINMIN_WEIGHTING_SHARED_COVARIANCE) return LINMIN_ERR_NOT_IMPLEMENTED;
+        return LINMIN_ERR_INVALID_ARGUMENT;
+    }
+    r->stream = (cudaStream_t)o->stream;
+    if (o->ldY != 0) { if (o->ldY < L) return LINMIN_ERR_INVALID_ARGUMENT; r->ldY = o->ldY; }
+    if (o->sigma_pixel_stride != 0) {
+        if (o->sigma_pixel_stride < L) return LINMIN_ERR_INVALID_ARGUMENT;
+        r->sstride = o->sigma_pixel_stride;
+    }
+    if (o->max_iter < 0 || o->max_iter > 255) return LINMIN_ERR_INVALID_ARGUMENT;
+    if (o->max_iter > 0) r->max_iter = o->max_iter;
+    if (o->gap_tol < 0.0f || o->feas_tol < 0.0f || std::isnan(o->gap_tol) || std::isnan(o->feas_tol))
+        return LINMIN_ERR_INVALID_ARGUMENT;
+    if (o->gap_tol > 0.0f) r->gap_tol = o->gap_tol;
+    if (o->feas_tol > 0.0f) r->feas_tol = o->feas_tol;
+    r->info = o->info_out;
+    return LINMIN_OK;
+}
+
+int check_sizes(int64_t N, int L, int R) {
+    if (N < 0 || L < 1 || R < 1) return LINMIN_ERR_INVALID_ARGUMENT;
+    if (R > LINMIN_MAX_R || L > LINMIN_MAX_L) return LINMIN_ERR_UNSUPPORTED_SIZE;
+    return LINMIN_OK;
+}
+
+LibView view_of(const linmin_library *lib) {
+    LibView v;
+    v.L = lib->L; v.R = lib->R; v.A = lib->A; v.Ac = lib->Ac; v.c = lib->c; v.Gc = lib->Gc;
+    v.G64 = lib->G64; v.gdmax = lib->gdmax;
+    return v;
+}
+
+// persistent grid: enough CTAs to fill every SM at the kernel's occupancy, never more than needed
+template <typename K>
+int persistent_grid(K kernel, int block, size_t smem, int sm_count, int64_t work_items, int items_per_cta) {
+    int occ = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, block, smem) != cudaSuccess || occ < 1) {
+        (void)cudaGetLastError();
+        occ = 1;
+    }
+    int64_t need = (work_items + items_per_cta - 1) / items_per_cta;
+    int64_t cap = (int64_t)sm_count * occ;
+    return (int)std::max<int64_t>(1, std::min(need, cap));
+}
+
+int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
+                 const Resolved &o, float *coeffs, float *csig, float *resid) {
+    const int L = lib->L, R = lib->R;
+    LibView lv = view_of(lib);
+    SolveParams prm;
+    prm.Y = Y; prm.sigma = sigma; prm.N = N; prm.ldY = o.ldY; prm.sigma_stride = o.sstride;
+    prm.has_sigma = sigma != nullptr;
+    prm.max_iter = o.max_iter; prm.gap_tol = o.gap_tol; prm.feas_tol = o.feas_tol;
+    prm.coeffs = coeffs; prm.coeff_sigma = csig; prm.resid = resid; prm.info = o.info;
+    int launches = 0;
+
+    // ---- K1: projection + IPLS
+    if (R == 32 && ipls_r32_supported(L)) {
+        CK(launch_ipls_r32(lv, prm, lib->sm_count, o.stream));
+        ++launches;
+    } else if (R <= 64) {
+        const int teams = 8, block = teams * 32;
+        size_t smem = teams * ipls_generic_team_floats(L, R) * sizeof(float);
+        CK(cudaFuncSetAttribute(ipls_generic_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int grid = persistent_grid(ipls_generic_kernel<32>, block, smem, lib->sm_count, N, teams);
+        ipls_generic_kernel<32><<<grid, block, smem, o.stream>>>(lv, prm);
+        CK(cudaGetLastError());
+        ++launches;
+    } else {
+        const int block = 256;
+        size_t smem = ipls_generic_team_floats(L, R) * sizeof(float);
+        CK(cudaFuncSetAttribute(ipls_generic_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int grid = persistent_grid(ipls_generic_kernel<256>, block, smem, lib->sm_count, N, 1);
+        ipls_generic_kernel<256><<<grid, block, smem, o.stream>>>(lv, prm);
+        CK(cudaGetLastError());
+        ++launches;
+    }
+    // ---- K2: exact finish + uncertainty + residual
+    {
+        const int KMAX = R <= 32 ? R : 64;
+        size_t per_warp = (finish_warp_bytes(L, R, KMAX) + 15) & ~(size_t)15;
+        int warps = (int)std::min<size_t>(8, (200 * 1024) / per_warp);
+        if (warps < 1) return LINMIN_ERR_UNSUPPORTED_SIZE;
+        size_t smem = per_warp * warps;
+        CK(cudaFuncSetAttribute(finish_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int grid = persistent_grid(finish_kernel, warps * 32, smem, lib->sm_count, N, warps);
+        finish_kernel<<<grid, warps * 32, smem, o.stream>>>(lv, prm, KMAX);
+        CK(cudaGetLastError());
+        ++launches;
+    }
+    lib->last_launches = launches;
+    return LINMIN_OK;
+}
+
+int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool A_on_host,
+                        linmin_library **out) {
+    *out = nullptr;
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    linmin_library *lib = new (std::nothrow) linmin_library();
+    if (!lib) return LINMIN_ERR_OUT_OF_MEMORY;
+    lib->L = L; lib->R = R; lib->device = dev; lib->stream = stream;
+    int rc = LINMIN_OK;
+    int *flags = nullptr;
+    std::vector<float> hG((size_t)R * R);
+    int hflags = 0;
+    auto fail = [&](int code) {
+        if (flags) cudaFreeAsync(flags, stream);
+        linmin_library_destroy(lib);
+        return code;
+    };
+#define CKF(call)                                                 \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) { (void)cudaGetLastError(); return fail(cuda_status(e__)); } \
+    } while (0)
+    CKF(cudaDeviceGetAttribute(&lib->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    const size_t LR = (size_t)L * R, RR = (size_t)R * R;
+    CKF(cudaMallocAsync((void **)&lib->A, LR * sizeof(float), stream));
+    CKF(cudaMallocAsync((void **)&lib->Ac, LR * sizeof(float), stream));
+    CKF(cudaMallocAsync((void **)&lib->c, (size_t)L * sizeof(float), stream));
+    CKF(cudaMallocAsync((void **)&lib->Gc, RR * sizeof(float), stream));
+    CKF(cudaMallocAsync((void **)&lib->G64, RR * sizeof(double), stream));
+    CKF(cudaMallocAsync((void **)&flags, sizeof(int), stream));
+    CKF(cudaMemsetAsync(flags, 0, sizeof(int), stream));
+    CKF(cudaMemcpyAsync(lib->A, A, LR * sizeof(float), A_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, stream));
+    {
+        int block = 256, grid = (L * 32 + block - 1) / block;
+        center_library_kernel<<<grid, block, 0, stream>>>(lib->A, L, R, lib->Ac, lib->c, flags);
+        CKF(cudaGetLastError());
+        grid = (int)((RR + block - 1) / block);
+        gram_kernel<<<grid, block, 0, stream>>>(lib->A, lib->Ac, L, R, lib->G64, lib->Gc);
+        CKF(cudaGetLastError());
+    }
+    CKF(cudaMemcpyAsync(hG.data(), lib->Gc, RR * sizeof(float), cudaMemcpyDeviceToHost, stream));
+    CKF(cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, stream));
+    CKF(cudaStreamSynchronize(stream));
+    cudaFreeAsync(flags, stream);
+    flags = nullptr;
+    if (hflags & 1) return fail(LINMIN_ERR_LIBRARY_NONFINITE);
+    float gd = 0.0f;
+    for (int i = 0; i < R; ++i) gd = std::max(gd, hG[(size_t)i * R + i]);
+    if (!(gd > 0.0f)) gd = 1.0f;   // all endmembers identical: any point of the simplex is optimal
+    lib->gdmax = gd;
+    if (R > L) rc = LINMIN_WARN_RANK_DEFICIENT;
+    *out = lib;
+    return rc;
+#undef CKF
+}
+
+}  // namespace
+
+extern "C" {
+
+int linmin_version(void) { return LINMIN_VERSION; }
+
+const char *linmin_strerror(int code) {
+    switch (code) {
+        case LINMIN_OK: return "ok";
+        case LINMIN_ERR_INVALID_ARGUMENT: return "invalid argument";
+        case LINMIN_ERR_UNSUPPORTED_SIZE: return "unsupported size (R > 256 or L > 512)";
+        case LINMIN_ERR_NOT_IMPLEMENTED: return "option not implemented";
+        case LINMIN_ERR_CUDA: return "CUDA runtime error (no device, or a failed call)";
+        case LINMIN_ERR_OUT_OF_MEMORY: return "out of device memory";
+        case LINMIN_ERR_LIBRARY_NONFINITE: return "library A contains a non-finite value";
+        case LINMIN_WARN_RANK_DEFICIENT: return "warning: R > L, the minimiser may be non-unique";
+        default: return "unknown status code";
+    }
+}
+
+int linmin_library_create(const float *A, int32_t L, int32_t R, const linmin_opts *opts, linmin_library **lib) {
+    if (!lib) return LINMIN_ERR_INVALID_ARGUMENT;
+    *lib = nullptr;
+    if (!A) return LINMIN_ERR_INVALID_ARGUMENT;
+    int rc = check_sizes(0, L, R);
+    if (rc != LINMIN_OK) return rc;
+    cudaStream_t stream = nullptr;
+    if (opts) {
+        if (opts->struct_size != sizeof(linmin_opts)) return LINMIN_ERR_INVALID_ARGUMENT;
+        stream = (cudaStream_t)opts->stream;
+    }
+    return library_create_impl(A, L, R, stream, false, lib);
+}
+
+void linmin_library_destroy(linmin_library *lib) {
+    if (!lib) return;
+    cudaStream_t s = lib->stream;
+    if (lib->A) cudaFreeAsync(lib->A, s);
+    if (lib->Ac) cudaFreeAsync(lib->Ac, s);
+    if (lib->c) cudaFreeAsync(lib->c, s);
+    if (lib->Gc) cudaFreeAsync(lib->Gc, s);
+    if (lib->G64) cudaFreeAsync(lib->G64, s);
+    (void)cudaGetLastError();
+    delete lib;
+}
+
+int linmin_library_last_launches(const linmin_library *lib) { return lib ? lib->last_launches : 0; }
+
+int linmin_unmix_lib(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
+                     const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out, float *resid_out) {
+    if (!lib) return LINMIN_ERR_INVALID_ARGUMENT;
+    if (N < 0) return LINMIN_ERR_INVALID_ARGUMENT;
+    Resolved o;
+    int rc = resolve_opts(opts, lib->L, &o);
+    if (rc != LINMIN_OK) return rc;
+    if (N == 0) { lib->last_launches = 0; return LINMIN_OK; }
+    if (!Y || !coeffs_out) return LINMIN_ERR_INVALID_ARGUMENT;
+    return launch_solve(lib, Y, sigma, N, o, coeffs_out, coeff_sigma_out, resid_out);
+}
+
+int linmin_unmix(const float *A, const float *Y, const float *sigma, int64_t N, int32_t L, int32_t R,
+                 const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out, float *resid_out) {
+    int rc = check_sizes(N, L, R);
+    if (rc != LINMIN_OK) return rc;
+    if (!A) return LINMIN_ERR_INVALID_ARGUMENT;
+    Resolved o;
+    rc = resolve_opts(opts, L, &o);
+    if (rc != LINMIN_OK) return rc;
+    if (N > 0 && (!Y || !coeffs_out)) return LINMIN_ERR_INVALID_ARGUMENT;
+    linmin_library *lib = nullptr;
+    int wrc = library_create_impl(A, L, R, o.stream, false, &lib);
+    if (wrc < 0) return wrc;
+    rc = LINMIN_OK;
+    if (N > 0) rc = launch_solve(lib, Y, sigma, N, o, coeffs_out, coeff_sigma_out, resid_out);
+    linmin_library_destroy(lib);   // stream-ordered frees: safe while the kernels are still queued
+    return rc != LINMIN_OK ? rc : wrc;
+}
+
+int linmin_unmix_host(const float *A, const float *Y, const float *sigma, int64_t N, int32_t L, int32_t R,
+                      const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out, float *resid_out) {
+    int rc = check_sizes(N, L, R);
+    if (rc != LINMIN_OK) return rc;
+    if (!A) return LINMIN_ERR_INVALID_ARGUMENT;
+    Resolved o;
+    rc = resolve_opts(opts, L, &o);
+    if (rc != LINMIN_OK) return rc;
+    if (N > 0 && (!Y || !coeffs_out)) return LINMIN_ERR_INVALID_ARGUMENT;
+
+    const int NBUF = 3;
+    cudaStream_t st[NBUF] = {nullptr, nullptr, nullptr};
+    float *dY[NBUF] = {}, *dS[NBUF] = {}, *dC[NBUF] = {}, *dCS[NBUF] = {}, *dR[NBUF] = {};
+    int32_t *dI[NBUF] = {};
+    float *dSshared = nullptr;
+    linmin_library *lib = nullptr;
+    int wrc = LINMIN_OK;
+    int64_t chunk = std::min<int64_t>(N, (int64_t)1 << 18);
+    auto cleanup = [&]() {
+        for (int b = 0; b < NBUF; ++b) {
+            if (st[b]) cudaStreamSynchronize(st[b]);
+            cudaFree(dY[b]); cudaFree(dS[b]); cudaFree(dC[b]); cudaFree(dCS[b]); cudaFree(dR[b]); cudaFree(dI[b]);
+            if (st[b]) cudaStreamDestroy(st[b]);
+        }
+        cudaFree(dSshared);
+        if (lib) { cudaStreamSynchronize(lib->stream); linmin_library_destroy(lib); }
+        (void)cudaGetLastError();
+    };
+#define CKH(call)                                                                   \
+    do {                                                                            \
+        cudaError_t e__ = (call);                                                   \
+        if (e__ != cudaSuccess) { (void)cudaGetLastError(); cleanup(); return cuda_status(e__); } \
+    } while (0)
+    wrc = library_create_impl(A, L, R, nullptr, true, &lib);
+    if (wrc < 0) { lib = nullptr; return wrc; }
+    if (N == 0) { cleanup(); return wrc; }
+    const bool per_pixel_sigma = sigma && o.sstride != 0;
+    if (sigma && !per_pixel_sigma) {
+        CKH(cudaMalloc((void **)&dSshared, (size_t)L * sizeof(float)));
+        CKH(cudaMemcpy(dSshared, sigma, (size_t)L * sizeof(float), cudaMemcpyHostToDevice));
+    }
+    for (int b = 0; b < NBUF; ++b) {
+        CKH(cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking));
+        CKH(cudaMalloc((void **)&dY[b], (size_t)chunk * L * sizeof(float)));
+        if (per_pixel_sigma) CKH(cudaMalloc((void **)&dS[b], (size_t)chunk * L * sizeof(float)));
+        CKH(cudaMalloc((void **)&dC[b], (size_t)chunk * R * sizeof(float)));
+        if (coeff_sigma_out) CKH(cudaMalloc((void **)&dCS[b], (size_t)chunk * R * sizeof(float)));
+        if (resid_out) CKH(cudaMalloc((void **)&dR[b], (size_t)chunk * sizeof(float)));
+        if (o.info) CKH(cudaMalloc((void **)&dI[b], (size_t)chunk * sizeof(int32_t)));
+    }
+    int bi = 0;
+    for (int64_t p0 = 0; p0 < N; p0 += chunk, bi = (bi + 1) % NBUF) {
+        int64_t n = std::min(chunk, N - p0);
+        cudaStream_t s = st[bi];
+        // stream order makes reuse of buffer set `bi` safe: its previous D2H copies precede these H2D
+        CKH(cudaMemcpy2DAsync(dY[bi], (size_t)L * sizeof(float), Y + p0 * o.ldY, (size_t)o.ldY * sizeof(float),
+                              (size_t)L * sizeof(float), (size_t)n, cudaMemcpyHostToDevice, s));
+        if (per_pixel_sigma)
+            CKH(cudaMemcpy2DAsync(dS[bi], (size_t)L * sizeof(float), sigma + p0 * o.sstride,
+                                  (size_t)o.sstride * sizeof(float), (size_t)L * sizeof(float), (size_t)n,
+                                  cudaMemcpyHostToDevice, s));
+        Resolved oc = o;
+        oc.stream = s; oc.ldY = L; oc.sstride = per_pixel_sigma ? L : 0; oc.info = dI[bi];
+        const float *sg = per_pixel_sigma ? dS[bi] : dSshared;
+        rc = launch_solve(lib, dY[bi], sg, n, oc, dC[bi], dCS[bi], dR[bi]);
+        if (rc != LINMIN_OK) { cleanup(); return rc; }
+        CKH(cudaMemcpyAsync(coeffs_out + p0 * R, dC[bi], (size_t)n * R * sizeof(float), cudaMemcpyDeviceToHost, s));
+        if (coeff_sigma_out)
+            CKH(cudaMemcpyAsync(coeff_sigma_out + p0 * R, dCS[bi], (size_t)n * R * sizeof(float), cudaMemcpyDeviceToHost, s));
+        if (resid_out)
+            CKH(cudaMemcpyAsync(resid_out + p0, dR[bi], (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s));
+        if (o.info)
+            CKH(cudaMemcpyAsync(o.info + p0, dI[bi], (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    }
+    for (int b = 0; b < NBUF; ++b) CKH(cudaStreamSynchronize(st[b]));
+    cleanup();
+    return wrc;
+#undef CKH
+}
+
+}  // extern "C"

@@ -1,0 +1,283 @@
+"""Thin ctypes binding over liblinmin.so (include/linmin.h).  Argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/; this module allocates nothing but the
+output tensors (PyTorch is used for device memory and streams) and never falls back to a CPU or
+PyTorch implementation: if the library or a CUDA device is missing, calls raise.
+Function names mirror the C ABI: unmix, unmix_lib, unmix_host, library_create, library_destroy.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblinmin.so")
+
+OK = 0
+ERR_INVALID_ARGUMENT = -1
+ERR_UNSUPPORTED_SIZE = -2
+ERR_NOT_IMPLEMENTED = -3
+ERR_CUDA = -4
+ERR_OUT_OF_MEMORY = -5
+ERR_LIBRARY_NONFINITE = -6
+WARN_RANK_DEFICIENT = 1
+
+INFO_CONVERGED = 0x01
+INFO_MAX_ITER = 0x02
+INFO_NONFINITE_INPUT = 0x04
+INFO_CHOL_REGULARISED = 0x08
+INFO_FINISH_FALLBACK = 0x10
+INFO_BAD_SIGMA = 0x20
+
+EXPORTS = ["linmin_version", "linmin_strerror", "linmin_library_create", "linmin_library_destroy",
+           "linmin_library_last_launches", "linmin_unmix_lib", "linmin_unmix", "linmin_unmix_host"]
+
+
+class LinminOpts(ctypes.Structure):
+    _fields_ = [("struct_size", ctypes.c_uint32), ("stream", ctypes.c_void_p),
+                ("ldY", ctypes.c_int64), ("sigma_pixel_stride", ctypes.c_int64),
+                ("constraint", ctypes.c_int32), ("weighting", ctypes.c_int32),
+                ("max_iter", ctypes.c_int32), ("gap_tol", ctypes.c_float),
+                ("feas_tol", ctypes.c_float), ("info_out", ctypes.c_void_p),
+                ("deterministic", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+class LinminError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"linmin error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """Load liblinmin.so (built in-tree by paper_1402_2518_b200.build).  Fails loudly if missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_1402_2518_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = ctypes.CDLL(LIB_PATH)
+        P, I64, I32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32
+        lib.linmin_version.restype = ctypes.c_int
+        lib.linmin_strerror.restype = ctypes.c_char_p
+        lib.linmin_strerror.argtypes = [ctypes.c_int]
+        lib.linmin_library_create.argtypes = [P, I32, I32, ctypes.POINTER(LinminOpts), ctypes.POINTER(P)]
+        lib.linmin_library_destroy.argtypes = [P]
+        lib.linmin_library_destroy.restype = None
+        lib.linmin_library_last_launches.argtypes = [P]
+        lib.linmin_unmix_lib.argtypes = [P, P, P, I64, ctypes.POINTER(LinminOpts), P, P, P]
+        lib.linmin_unmix.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
+        lib.linmin_unmix_host.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
+        _lib = lib
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return load().linmin_strerror(int(code)).decode()
+
+
+def version() -> int:
+    return int(load().linmin_version())
+
+
+def _check(code: int) -> int:
+    if code < 0:
+        raise LinminError(code, strerror(code))
+    return code
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _dev_ptr(t, name, dtype=None):
+    torch = _torch()
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    if t.dtype != (dtype or torch.float32):
+        raise ValueError(f"{name} must be {dtype or torch.float32}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _make_opts(stream=None, ldY=0, sigma_pixel_stride=0, constraint=0, weighting=0, max_iter=0,
+               gap_tol=0.0, feas_tol=0.0, info_ptr=None) -> LinminOpts:
+    o = LinminOpts()
+    o.struct_size = ctypes.sizeof(LinminOpts)
+    o.stream = stream
+    o.ldY = ldY
+    o.sigma_pixel_stride = sigma_pixel_stride
+    o.constraint = constraint
+    o.weighting = weighting
+    o.max_iter = max_iter
+    o.gap_tol = gap_tol
+    o.feas_tol = feas_tol
+    o.info_out = info_ptr
+    o.deterministic = 1
+    return o
+
+
+def _sigma_stride(sigma, N, L):
+    if sigma is None:
+        return 0
+    if sigma.dim() == 1:
+        if sigma.shape[0] != L:
+            raise ValueError("shared sigma must have L entries")
+        return 0
+    if tuple(sigma.shape) != (N, L):
+        raise ValueError("per-pixel sigma must be (N, L)")
+    return L
+
+
+class Library:
+    """linmin_library handle: once-per-library precompute kept on the device."""
+
+    def __init__(self, A):
+        torch = _torch()
+        if A.dim() != 2:
+            raise ValueError("A must be (L, R)")
+        self.L, self.R = int(A.shape[0]), int(A.shape[1])
+        self._h = ctypes.c_void_p()
+        self.device = A.device
+        with torch.cuda.device(A.device):
+            o = _make_opts(stream=torch.cuda.current_stream().cuda_stream)
+            self.status = _check(load().linmin_library_create(_dev_ptr(A, "A"), self.L, self.R,
+                                                              ctypes.byref(o), ctypes.byref(self._h)))
+
+    def last_launches(self) -> int:
+        return int(load().linmin_library_last_launches(self._h))
+
+    def destroy(self):
+        if self._h:
+            load().linmin_library_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def library_create(A) -> Library:
+    return Library(A)
+
+
+def library_destroy(lib: Library) -> None:
+    lib.destroy()
+
+
+def _alloc_outputs(N, R, device, want_sigma, want_resid, want_info, out):
+    torch = _torch()
+    out = dict(out or {})
+    coeffs = out.get("coeffs")
+    if coeffs is None:
+        coeffs = torch.empty((N, R), dtype=torch.float32, device=device)
+    csig = out.get("coeff_sigma")
+    if csig is None and want_sigma:
+        csig = torch.empty((N, R), dtype=torch.float32, device=device)
+    resid = out.get("resid")
+    if resid is None and want_resid:
+        resid = torch.empty((N,), dtype=torch.float32, device=device)
+    info = out.get("info")
+    if info is None and want_info:
+        info = torch.empty((N,), dtype=torch.int32, device=device)
+    return coeffs, csig, resid, info
+
+
+def unmix_lib(lib: Library, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=True,
+              out: Optional[dict] = None, max_iter=0, gap_tol=0.0, feas_tol=0.0, constraint=0,
+              weighting=0):
+    """linmin_unmix_lib.  Y (N, L) CUDA float32 (rows may be strided); returns
+    (coeffs, coeff_sigma, resid, info, status); enqueued on the current stream, not synchronised."""
+    torch = _torch()
+    if Y.dim() != 2 or Y.shape[1] != lib.L:
+        raise ValueError("Y must be (N, L)")
+    N = int(Y.shape[0])
+    ldY = int(Y.stride(0)) if N > 1 else lib.L
+    if Y.stride(1) != 1 and N > 0:
+        raise ValueError("spectra must be contiguous along channels")
+    coeffs, csig, resid, info = _alloc_outputs(N, lib.R, Y.device, want_sigma, want_resid, want_info, out)
+    with torch.cuda.device(Y.device):
+        o = _make_opts(stream=torch.cuda.current_stream().cuda_stream, ldY=ldY,
+                       sigma_pixel_stride=_sigma_stride(sigma, N, lib.L), constraint=constraint,
+                       weighting=weighting, max_iter=max_iter, gap_tol=gap_tol, feas_tol=feas_tol,
+                       info_ptr=None if info is None else info.data_ptr())
+        yp = ctypes.c_void_p(Y.data_ptr()) if N > 0 else None
+        if N > 0 and (not Y.is_cuda or Y.dtype != torch.float32):
+            raise ValueError("Y must be a CUDA float32 tensor")
+        st = _check(load().linmin_unmix_lib(lib._h, yp, _dev_ptr(sigma, "sigma"), N, ctypes.byref(o),
+                                            _dev_ptr(coeffs, "coeffs"), _dev_ptr(csig, "coeff_sigma"),
+                                            _dev_ptr(resid, "resid")))
+    return coeffs, csig, resid, info, st
+
+
+def unmix(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=True,
+          out: Optional[dict] = None, max_iter=0, gap_tol=0.0, feas_tol=0.0, constraint=0, weighting=0):
+    """linmin_unmix (one-shot: precompute + solve).  All tensors CUDA float32."""
+    torch = _torch()
+    L, R = int(A.shape[0]), int(A.shape[1])
+    N = int(Y.shape[0])
+    coeffs, csig, resid, info = _alloc_outputs(N, R, A.device, want_sigma, want_resid, want_info, out)
+    with torch.cuda.device(A.device):
+        o = _make_opts(stream=torch.cuda.current_stream().cuda_stream, ldY=0,
+                       sigma_pixel_stride=_sigma_stride(sigma, N, L), constraint=constraint,
+                       weighting=weighting, max_iter=max_iter, gap_tol=gap_tol, feas_tol=feas_tol,
+                       info_ptr=None if info is None else info.data_ptr())
+        st = _check(load().linmin_unmix(_dev_ptr(A, "A"), _dev_ptr(Y, "Y") if N > 0 else None,
+                                        _dev_ptr(sigma, "sigma"), N, L, R, ctypes.byref(o),
+                                        _dev_ptr(coeffs, "coeffs"), _dev_ptr(csig, "coeff_sigma"),
+                                        _dev_ptr(resid, "resid")))
+    return coeffs, csig, resid, info, st
+
+
+def unmix_host(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=False,
+               out: Optional[dict] = None, max_iter=0, gap_tol=0.0, feas_tol=0.0):
+    """linmin_unmix_host: numpy arrays or CPU tensors (pinned memory gives full copy bandwidth).
+    Blocks until the outputs are complete.  Returns (coeffs, coeff_sigma, resid, info, status) as
+    CPU tensors (pinned when freshly allocated)."""
+    torch = _torch()
+
+    def as_cpu(x, name):
+        if x is None:
+            return None
+        t = torch.as_tensor(x)
+        if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+            raise ValueError(f"{name} must be a contiguous CPU float32 array")
+        return t
+
+    A, Y, sigma = as_cpu(A, "A"), as_cpu(Y, "Y"), as_cpu(sigma, "sigma")
+    L, R = int(A.shape[0]), int(A.shape[1])
+    N = int(Y.shape[0])
+    out = dict(out or {})
+    pin = torch.cuda.is_available()
+
+    def host_empty(shape, dtype):
+        return torch.empty(shape, dtype=dtype, pin_memory=pin)
+
+    coeffs = out.get("coeffs") if out.get("coeffs") is not None else host_empty((N, R), torch.float32)
+    csig = out.get("coeff_sigma")
+    if csig is None and want_sigma:
+        csig = host_empty((N, R), torch.float32)
+    resid = out.get("resid")
+    if resid is None and want_resid:
+        resid = host_empty((N,), torch.float32)
+    info = out.get("info")
+    if info is None and want_info:
+        info = host_empty((N,), torch.int32)
+    o = _make_opts(ldY=0, sigma_pixel_stride=_sigma_stride(sigma, N, L), max_iter=max_iter,
+                   gap_tol=gap_tol, feas_tol=feas_tol, info_ptr=None if info is None else info.data_ptr())
+
+    def hp(t):
+        return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+    st = _check(load().linmin_unmix_host(hp(A), hp(Y) if N > 0 else None, hp(sigma), N, L, R,
+                                         ctypes.byref(o), hp(coeffs), hp(csig), hp(resid)))
+    return coeffs, csig, resid, info, st

@@ -1,0 +1,80 @@
+"""Shared parity checks: CUDA path (through the C ABI) vs the fp64 oracle, on identical inputs.
+
+Tolerances are north_star's (BASELINE.json), read as in DESIGN.md R10/R12:
+  max |a_gpu - a*| <= 1e-4, |sum a - 1| <= 1e-5, a >= -1e-6,
+  |F(a_gpu) - F*| <= 1e-5 max(F*, 1e-12 ||y||^2) with F re-evaluated here in fp64,
+  resid within 1e-5 relative (same floor), coeff_sigma within 1 % relative (+1e-7 absolute) where the
+  supports agree; where they differ (ties, R10) the GPU value is compared with reading R3 evaluated
+  in numpy ON THE GPU's support, and the number of such pixels must stay below 0.5 %.
+"""
+import numpy as np
+
+
+def sigma_reference_on_support(A64, F, sig):
+    """Reading R3 written out with numpy for a given support (independent of oracle/ and of csrc/)."""
+    out = np.zeros(A64.shape[1])
+    F = np.asarray(F)
+    if len(F) <= 1:
+        return out
+    AF = A64[:, F]
+    K = np.linalg.inv(AF.T @ AF)
+    one = np.ones(len(F))
+    H = K - np.outer(K @ one, one @ K) / (one @ K @ one)
+    J = H @ AF.T
+    out[F] = np.sqrt((J ** 2) @ (sig.astype(np.float64) ** 2))
+    return out
+
+
+def check_parity(A, Y, sigma, gpu, ora, label="", require_unique=True):
+    """gpu: dict(coeffs, coeff_sigma, resid) numpy float32 arrays for the SAME pixels as ora."""
+    A64 = A.astype(np.float64)
+    Y64 = Y.astype(np.float64)
+    a = gpu["coeffs"].astype(np.float64)
+    N, R = a.shape
+    L = A.shape[0]
+    assert np.isfinite(a).all(), label
+    # feasibility
+    assert np.abs(a.sum(1) - 1.0).max() <= 1e-5, (label, np.abs(a.sum(1) - 1.0).max())
+    assert a.min() >= -1e-6, (label, a.min())
+    # objective (R12)
+    Fg = ((Y64 - a @ A64.T) ** 2).sum(1)
+    Fo = ((Y64 - ora.coeffs @ A64.T) ** 2).sum(1)
+    floor = 1e-12 * (Y64 ** 2).sum(1)
+    rel = np.abs(Fg - Fo) / np.maximum(Fo, floor)
+    assert rel.max() <= 1e-5, (label, "objective", rel.max(), int(rel.argmax()))
+    # coefficients: where the minimiser is unique (R9)
+    sing = np.linalg.svd(A64, compute_uv=False)
+    unique = ora.rank_margin > 1e-6 * sing[0]
+    if require_unique:
+        assert unique.mean() > 0.99, (label, unique.mean())
+    da = np.abs(a - ora.coeffs).max(1)
+    assert da[unique].max() <= 1e-4, (label, "coeffs", da[unique].max(), int(np.argmax(np.where(unique, da, 0))))
+    stats = dict(max_da=float(da[unique].max()), max_rel_obj=float(rel.max()), n_nonunique=int((~unique).sum()))
+    # residual
+    if gpu.get("resid") is not None:
+        rg = gpu["resid"].astype(np.float64)
+        rr = np.abs(rg - ora.resid) / np.maximum(ora.resid, np.sqrt(floor / L))
+        assert rr.max() <= 1e-5, (label, "resid", rr.max())
+        stats["max_rel_resid"] = float(rr.max())
+    # uncertainties
+    if gpu.get("coeff_sigma") is not None:
+        sg = gpu["coeff_sigma"].astype(np.float64)
+        Fg_sup = a > 0
+        Fo_sup = ora.coeffs > 0
+        same = (Fg_sup == Fo_sup).all(1)
+        err = np.abs(sg - ora.coeff_sigma) - (0.01 * ora.coeff_sigma + 1e-7)
+        assert err[same & unique].max() <= 0, (label, "sigma", err[same & unique].max())
+        ties = np.nonzero(~same & unique)[0]
+        assert len(ties) <= max(2, 0.005 * N), (label, "support mismatches", len(ties))
+        for p in ties:
+            # the differing members must be marginal (tiny coefficient on either side)
+            diff = Fg_sup[p] ^ Fo_sup[p]
+            assert max(a[p][diff].max(), ora.coeffs[p][diff].max()) < 1e-4, (label, p)
+            sp = sigma[p] if sigma.ndim == 2 else sigma
+            ref = sigma_reference_on_support(A64, np.nonzero(Fg_sup[p])[0], sp)
+            assert (np.abs(sg[p] - ref) <= 0.01 * ref + 1e-7).all(), (label, "tie sigma", p)
+        stats["n_support_ties"] = int(len(ties))
+        m = same & unique
+        pos = ora.coeff_sigma[m] > 1e-6
+        stats["max_rel_sigma"] = float((np.abs(sg[m] - ora.coeff_sigma[m])[pos] / ora.coeff_sigma[m][pos]).max()) if pos.any() else 0.0
+    return stats

@@ -1,0 +1,222 @@
+"""-m gpu: the CUDA path, called through the C ABI (ctypes binding), against the fp64 oracle on the
+same seeded inputs.  Tolerances: tests/parity.py (north_star).  Nothing here reads /root/reference."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def lm():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1402_2518_b200 import build, linmin
+    build.build_library()
+    linmin.load()
+    return linmin
+
+
+def run_gpu(lm, A, Y, sigma, **kw):
+    dev = torch.device("cuda:0")
+    At = torch.from_numpy(A).to(dev)
+    Yt = torch.from_numpy(Y).to(dev)
+    st = None if sigma is None else torch.from_numpy(sigma).to(dev)
+    c, s, r, info, status = lm.unmix(At, Yt, st, **kw)
+    torch.cuda.synchronize()
+    return dict(coeffs=c.cpu().numpy(), coeff_sigma=None if s is None else s.cpu().numpy(),
+                resid=None if r is None else r.cpu().numpy(), info=info.cpu().numpy(), status=status)
+
+
+def subsample(g, sel):
+    return {k: (v[sel] if isinstance(v, np.ndarray) else v) for k, v in g.items()}
+
+
+# ------------------------------------------------------------------ the five configs
+@pytest.mark.parametrize("name,stride", [("tiny", 1), ("omega", 1), ("crism", 16), ("stress", 32)])
+def test_config_parity(lm, name, stride):
+    """Full-size configs 0-3 through the launch configuration bench.py uses; the oracle checks every
+    pixel (configs 0-1) or every `stride`-th pixel (configs 2-3)."""
+    import oracle
+    from paper_1402_2518_b200.synth import make_workload
+    from parity import check_parity
+    w = make_workload(name)
+    g = run_gpu(lm, w.A, w.Y, w.sigma)
+    sel = np.arange(0, w.N, stride)
+    ora = oracle.solve(w.A, w.Y[sel], w.sigma[sel])
+    stats = check_parity(w.A, w.Y[sel], w.sigma[sel], subsample(g, sel), ora, label=name,
+                         require_unique=(name != "stress"))
+    info = g["info"]
+    assert ((info & lm.INFO_NONFINITE_INPUT) == 0).all()
+    assert ((info & lm.INFO_FINISH_FALLBACK) == 0).mean() > 0.9999
+    # exact zeros off the support, support size reported
+    assert (((g["coeffs"] > 0).sum(1)) == ((info >> 24) & 0xff)).all()
+    if name == "crism":      # pixels drawn on a simplex face are reported separately
+        face = w.face[sel]
+        da = np.abs(subsample(g, sel)["coeffs"] - ora.coeffs).max(1)
+        assert da[face].max() <= 1e-4
+    print(name, stats, "iters mean", ((info >> 8) & 0xff).mean(), "pivots mean", ((info >> 16) & 0xff).mean())
+
+
+def test_throughput_config_sampled(lm):
+    """Config 4 (a stack of OMEGA-like cubes): 8 cubes = 1,048,576 pixels on the GPU, every 64th
+    pixel against the oracle."""
+    import oracle
+    from paper_1402_2518_b200.synth import make_workload
+    from parity import check_parity
+    w = make_workload("throughput", n_cubes=8)
+    g = run_gpu(lm, w.A, w.Y, w.sigma)
+    sel = np.arange(0, w.N, 64)
+    ora = oracle.solve(w.A, w.Y[sel], w.sigma[sel])
+    print(check_parity(w.A, w.Y[sel], w.sigma[sel], subsample(g, sel), ora, label="throughput"))
+
+
+# ------------------------------------------------------------------ interfaces and edge cases
+def test_library_handle_strides_shared_sigma_and_host_path(lm):
+    import oracle
+    from paper_1402_2518_b200.synth import make_workload
+    from parity import check_parity
+    w = make_workload("omega", N=1003)          # ragged: not a multiple of any tile size
+    dev = torch.device("cuda:0")
+    lib = lm.library_create(torch.from_numpy(w.A).to(dev))
+    assert lib.status == 0
+    # strided Y (ldY > L), shared sigma vector
+    Ypad = torch.zeros((w.N, w.L + 5), device=dev)
+    Ypad[:, :w.L] = torch.from_numpy(w.Y).to(dev)
+    sig = w.sigma[0].copy()
+    c, s, r, info, st = lm.unmix_lib(lib, Ypad[:, :w.L], torch.from_numpy(sig).to(dev))
+    torch.cuda.synchronize()
+    ora = oracle.solve(w.A, w.Y, sig)
+    g = dict(coeffs=c.cpu().numpy(), coeff_sigma=s.cpu().numpy(), resid=r.cpu().numpy())
+    check_parity(w.A, w.Y, sig, g, ora, label="strided/shared")
+    assert lib.last_launches() >= 2
+    # sigma == NULL -> noise amplification factors (sigma == 1)
+    c1, s1, r1, _, _ = lm.unmix_lib(lib, torch.from_numpy(w.Y).to(dev), None)
+    torch.cuda.synchronize()
+    ora1 = oracle.solve(w.A, w.Y, None)
+    check_parity(w.A, w.Y, np.ones(w.L, np.float32),
+                 dict(coeffs=c1.cpu().numpy(), coeff_sigma=s1.cpu().numpy(), resid=r1.cpu().numpy()), ora1, label="nosigma")
+    # outputs optional
+    c2, s2, r2, i2, _ = lm.unmix_lib(lib, torch.from_numpy(w.Y).to(dev), None, want_sigma=False, want_resid=False, want_info=False)
+    torch.cuda.synchronize()
+    assert s2 is None and r2 is None and i2 is None
+    assert torch.equal(c2, c1)
+    # host entry point: same kernels, host buffers -> identical bits
+    ch, sh, rh, ih, _ = lm.unmix_host(w.A, w.Y, w.sigma, want_info=True)
+    cd, sd, rd, idv, _ = lm.unmix_lib(lib, torch.from_numpy(w.Y).to(dev), torch.from_numpy(w.sigma).to(dev))
+    torch.cuda.synchronize()
+    assert np.array_equal(ch.numpy(), cd.cpu().numpy())
+    assert np.array_equal(sh.numpy(), sd.cpu().numpy())
+    assert np.array_equal(rh.numpy(), rd.cpu().numpy())
+    assert np.array_equal(ih.numpy(), idv.cpu().numpy())
+    lib.destroy()
+
+
+def test_empty_single_and_determinism(lm):
+    from paper_1402_2518_b200.synth import make_workload
+    w = make_workload("tiny", N=9)
+    g0 = run_gpu(lm, w.A, w.Y[:0], w.sigma[:0])
+    assert g0["coeffs"].shape == (0, 8)
+    g1 = run_gpu(lm, w.A, w.Y[:1], w.sigma[:1])
+    g9 = run_gpu(lm, w.A, w.Y, w.sigma)
+    g9b = run_gpu(lm, w.A, w.Y, w.sigma)
+    assert np.array_equal(g1["coeffs"][0], g9["coeffs"][0])       # independent of N / tiling
+    assert np.array_equal(g9["coeffs"], g9b["coeffs"])            # run-to-run deterministic
+    assert np.array_equal(g9["coeff_sigma"], g9b["coeff_sigma"])
+
+
+def test_degenerate_inputs(lm):
+    import oracle
+    from parity import check_parity
+    rng = np.random.default_rng(9)
+    L = 10
+    # R = 1
+    A1 = rng.uniform(0.1, 0.9, (L, 1)).astype(np.float32)
+    y = rng.uniform(0, 1, (3, L)).astype(np.float32)
+    g = run_gpu(lm, A1, y, np.full((3, L), 0.01, np.float32))
+    assert (g["coeffs"] == 1.0).all() and (g["coeff_sigma"] == 0).all()
+    r = y.astype(np.float64) - A1.astype(np.float64).T
+    np.testing.assert_allclose(g["resid"], np.sqrt((r ** 2).mean(1)), rtol=1e-6)
+    # R = 2: closed form of tests/test_oracle_pins.py::test_r2_closed_form
+    A2 = rng.uniform(0.1, 0.9, (L, 2)).astype(np.float32)
+    Y2 = rng.uniform(-0.2, 1.2, (64, L)).astype(np.float32)
+    g2 = run_gpu(lm, A2, Y2, None)
+    d = A2[:, 0].astype(np.float64) - A2[:, 1]
+    t = np.clip((Y2.astype(np.float64) - A2[:, 1]) @ d / (d @ d), 0, 1)
+    np.testing.assert_allclose(g2["coeffs"][:, 0], t, atol=1e-6)
+    # duplicate column (rank-deficient library): objective parity, twins sum to the unique answer
+    A = rng.uniform(0.1, 0.9, (L, 4)).astype(np.float32)
+    Ad = np.concatenate([A, A[:, :1]], axis=1)
+    a0 = np.array([0.5, 0.2, 0.3, 0.0])
+    Y = (A.astype(np.float64) @ a0 + 0.01 * rng.standard_normal((20, L))).astype(np.float32)
+    gd = run_gpu(lm, Ad, Y, None)
+    ou = oracle.solve(A, Y)
+    np.testing.assert_allclose(gd["coeffs"][:, 0] + gd["coeffs"][:, 4], ou.coeffs[:, 0], atol=1e-5)
+    np.testing.assert_allclose(gd["resid"], ou.resid, rtol=1e-5)
+    # R > L (LINMIN_WARN_RANK_DEFICIENT): objective parity only
+    Aw = rng.uniform(0.1, 0.9, (4, 6)).astype(np.float32)
+    Yw = rng.uniform(0.1, 0.9, (16, 4)).astype(np.float32)
+    gw = run_gpu(lm, Aw, Yw, None)
+    assert gw["status"] == lm.WARN_RANK_DEFICIENT
+    ow = oracle.solve(Aw, Yw)
+    Fg = ((Yw - gw["coeffs"].astype(np.float64) @ Aw.T.astype(np.float64)) ** 2).sum(1)
+    Fo = ((Yw - ow.coeffs @ Aw.T.astype(np.float64)) ** 2).sum(1)
+    assert (np.abs(Fg - Fo) <= 1e-5 * np.maximum(Fo, 1e-12 * (Yw.astype(np.float64) ** 2).sum(1))).all()
+    assert np.abs(gw["coeffs"].sum(1) - 1).max() <= 1e-5 and gw["coeffs"].min() >= 0
+    # NaN pixel and bad sigma: flagged, NaN outputs, neighbours untouched
+    Yn = Y.copy(); Yn[3, 2] = np.nan
+    S = np.full((20, L), 0.01, np.float32); S[5, 1] = 0.0
+    gn = run_gpu(lm, A, Yn, S)
+    gref = run_gpu(lm, A, Y, np.full((20, L), 0.01, np.float32))
+    assert np.isnan(gn["coeffs"][3]).all() and np.isnan(gn["resid"][3]) and (gn["info"][3] & lm.INFO_NONFINITE_INPUT)
+    assert np.isnan(gn["coeff_sigma"][5]).all() and (gn["info"][5] & lm.INFO_BAD_SIGMA)
+    assert np.array_equal(gn["coeffs"][5], gref["coeffs"][5])
+    assert np.array_equal(gn["coeffs"][4], gref["coeffs"][4]) and np.array_equal(gn["coeff_sigma"][4], gref["coeff_sigma"][4])
+    # non-finite library is refused
+    Ab = A.copy(); Ab[0, 0] = np.inf
+    with pytest.raises(lm.LinminError) as e:
+        run_gpu(lm, Ab, Y, None)
+    assert e.value.code == lm.ERR_LIBRARY_NONFINITE
+
+
+def test_scale_and_offset_invariance(lm):
+    """R13: relative stopping rules -> (cA, cy) gives the same coefficients; offset invariance (eq. 4)."""
+    from paper_1402_2518_b200.synth import make_workload
+    w = make_workload("omega", N=512)
+    g = run_gpu(lm, w.A, w.Y, w.sigma)
+    gs = run_gpu(lm, 4 * w.A, 4 * w.Y, 4 * w.sigma)
+    np.testing.assert_allclose(gs["coeffs"], g["coeffs"], atol=2e-6)
+    np.testing.assert_allclose(gs["resid"], 4 * g["resid"], rtol=1e-5)
+    it, its = (g["info"] >> 8) & 0xff, (gs["info"] >> 8) & 0xff
+    assert np.abs(it.astype(int) - its.astype(int)).max() <= 1
+    go = run_gpu(lm, w.A + np.float32(0.25), w.Y + np.float32(0.25), w.sigma)
+    np.testing.assert_allclose(go["coeffs"], g["coeffs"], atol=2e-5)
+
+
+@pytest.mark.parametrize("L,R", [(110, 36), (56, 36), (33, 5), (200, 100)])
+def test_odd_sizes(lm, L, R):
+    """The paper's own sizes (110 or 56 channels, 36 endmembers) and others."""
+    import oracle
+    from parity import check_parity
+    rng = np.random.default_rng(L * 1000 + R)
+    lam = np.linspace(1.0, 2.5, L)
+    cols = []
+    for _ in range(R - 2):
+        c0, c1 = rng.uniform(0.2, 0.6, 2)
+        s = c0 + (c1 - c0) * (lam - 1.0) / 1.5
+        for _ in range(rng.integers(1, 4)):
+            s = s * (1 - rng.uniform(0.05, 0.4) * np.exp(-0.5 * ((lam - rng.uniform(1.0, 2.5)) / rng.uniform(0.01, 0.06)) ** 2))
+        cols.append(s)
+    cols += [np.ones(L), (lam - 1.0) / 1.5]
+    A = np.stack(cols, 1).astype(np.float32)
+    N = 777
+    a0 = np.zeros((N, R))
+    for p in range(N):
+        k = rng.integers(1, 5)
+        a0[p, rng.choice(R, k, replace=False)] = rng.dirichlet(0.3 * np.ones(k))
+    sig = rng.uniform(0.002, 0.01, (N, L)).astype(np.float32)
+    Y = (a0 @ A.astype(np.float64).T + sig * rng.standard_normal((N, L))).astype(np.float32)
+    g = run_gpu(lm, A, Y, sig)
+    ora = oracle.solve(A, Y, sig)
+    print(check_parity(A, Y, sig, g, ora, label=f"L{L}R{R}", require_unique=False))
