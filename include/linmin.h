@@ -133,6 +133,14 @@ int linmin_unmix_host(const float *A, const float *Y, const float *sigma, int64_
 /* Number of kernel launches the last linmin_unmix_lib call on this handle enqueued (for reports). */
 int linmin_library_last_launches(const linmin_library *lib);
 
+/* Per-kernel timing for reports (bench.py's roofline): when enabled, linmin_unmix_lib brackets each
+ * of its kernels with CUDA events on the call's stream.  linmin_library_last_timing blocks until the
+ * last call's events have completed and returns the device time of the projection+IPLS kernel and of
+ * the finish/uncertainty/residual kernel in milliseconds.  Returns LINMIN_ERR_INVALID_ARGUMENT when
+ * timing is disabled or no call was made.  Not thread-safe per handle. */
+int linmin_library_enable_timing(linmin_library *lib, int enable);
+int linmin_library_last_timing(const linmin_library *lib, float *ipls_ms, float *finish_ms);
+
 const char *linmin_strerror(int code);
 int linmin_version(void);
 

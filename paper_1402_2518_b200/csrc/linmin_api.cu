@@ -26,6 +26,9 @@ struct linmin_library {
     double *G64 = nullptr;
     float gdmax = 0.0f;
     mutable int last_launches = 0;
+    bool timing = false;
+    mutable bool timed = false;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
 };
 
 namespace {
@@ -119,6 +122,7 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     prm.max_iter = o.max_iter; prm.gap_tol = o.gap_tol; prm.feas_tol = o.feas_tol;
     prm.coeffs = coeffs; prm.coeff_sigma = csig; prm.resid = resid; prm.info = o.info;
     int launches = 0;
+    if (lib->timing) CK(cudaEventRecord(lib->ev[0], o.stream));
 
     // ---- K1: projection + IPLS
     if (R == 32 && ipls_r32_supported(L)) {
@@ -141,6 +145,7 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
         CK(cudaGetLastError());
         ++launches;
     }
+    if (lib->timing) CK(cudaEventRecord(lib->ev[1], o.stream));
     // ---- K2: exact finish + uncertainty + residual
     {
         const int KMAX = R <= 32 ? R : 64;
@@ -154,6 +159,7 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
         CK(cudaGetLastError());
         ++launches;
     }
+    if (lib->timing) { CK(cudaEventRecord(lib->ev[2], o.stream)); lib->timed = true; }
     lib->last_launches = launches;
     return LINMIN_OK;
 }
@@ -256,11 +262,32 @@ void linmin_library_destroy(linmin_library *lib) {
     if (lib->c) cudaFreeAsync(lib->c, s);
     if (lib->Gc) cudaFreeAsync(lib->Gc, s);
     if (lib->G64) cudaFreeAsync(lib->G64, s);
+    for (int i = 0; i < 3; ++i) if (lib->ev[i]) cudaEventDestroy(lib->ev[i]);
     (void)cudaGetLastError();
     delete lib;
 }
 
 int linmin_library_last_launches(const linmin_library *lib) { return lib ? lib->last_launches : 0; }
+
+int linmin_library_enable_timing(linmin_library *lib, int enable) {
+    if (!lib) return LINMIN_ERR_INVALID_ARGUMENT;
+    if (enable && !lib->ev[0])
+        for (int i = 0; i < 3; ++i) CK(cudaEventCreate(&lib->ev[i]));
+    lib->timing = enable != 0;
+    lib->timed = false;
+    return LINMIN_OK;
+}
+
+int linmin_library_last_timing(const linmin_library *lib, float *ipls_ms, float *finish_ms) {
+    if (!lib || !lib->timing || !lib->timed) return LINMIN_ERR_INVALID_ARGUMENT;
+    CK(cudaEventSynchronize(lib->ev[2]));
+    float a = 0.0f, b = 0.0f;
+    CK(cudaEventElapsedTime(&a, lib->ev[0], lib->ev[1]));
+    CK(cudaEventElapsedTime(&b, lib->ev[1], lib->ev[2]));
+    if (ipls_ms) *ipls_ms = a;
+    if (finish_ms) *finish_ms = b;
+    return LINMIN_OK;
+}
 
 int linmin_unmix_lib(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
                      const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out, float *resid_out) {

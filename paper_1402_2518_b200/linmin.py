@@ -31,7 +31,8 @@ INFO_FINISH_FALLBACK = 0x10
 INFO_BAD_SIGMA = 0x20
 
 EXPORTS = ["linmin_version", "linmin_strerror", "linmin_library_create", "linmin_library_destroy",
-           "linmin_library_last_launches", "linmin_unmix_lib", "linmin_unmix", "linmin_unmix_host"]
+           "linmin_library_last_launches", "linmin_library_enable_timing", "linmin_library_last_timing",
+           "linmin_unmix_lib", "linmin_unmix", "linmin_unmix_host"]
 
 
 class LinminOpts(ctypes.Structure):
@@ -68,6 +69,8 @@ def load() -> ctypes.CDLL:
         lib.linmin_library_destroy.argtypes = [P]
         lib.linmin_library_destroy.restype = None
         lib.linmin_library_last_launches.argtypes = [P]
+        lib.linmin_library_enable_timing.argtypes = [P, ctypes.c_int]
+        lib.linmin_library_last_timing.argtypes = [P, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]
         lib.linmin_unmix_lib.argtypes = [P, P, P, I64, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_unmix.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_unmix_host.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
@@ -153,6 +156,15 @@ class Library:
 
     def last_launches(self) -> int:
         return int(load().linmin_library_last_launches(self._h))
+
+    def enable_timing(self, enable: bool = True) -> None:
+        _check(load().linmin_library_enable_timing(self._h, int(enable)))
+
+    def last_timing(self):
+        """(ipls_ms, finish_ms) of the last unmix_lib call; blocks until its kernels have finished."""
+        a, b = ctypes.c_float(), ctypes.c_float()
+        _check(load().linmin_library_last_timing(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return float(a.value), float(b.value)
 
     def destroy(self):
         if self._h:
