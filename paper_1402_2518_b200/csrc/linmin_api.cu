@@ -126,7 +126,11 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
 
     // ---- K1: projection + IPLS
     if (R == 32 && ipls_r32_supported(L)) {
-        CK(launch_ipls_r32(lv, prm, lib->sm_count, o.stream));
+        unsigned int *counter = nullptr;      // per call: the same handle may serve several streams
+        CK(cudaMallocAsync((void **)&counter, sizeof(unsigned int), o.stream));
+        cudaError_t e = launch_ipls_r32(lv, prm, lib->sm_count, counter, o.stream);
+        cudaFreeAsync(counter, o.stream);
+        CK(e);
         ++launches;
     } else if (R <= 64) {
         const int teams = 8, block = teams * 32;
