@@ -11,6 +11,7 @@
 
 #include "common.cuh"
 #include "finish.cuh"
+#include "finish_fast.cuh"
 #include "ipls_generic.cuh"
 #include "ipls_r32.cuh"
 #include "precompute.cuh"
@@ -125,12 +126,12 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     if (lib->timing) CK(cudaEventRecord(lib->ev[0], o.stream));
 
     // ---- K1: projection + IPLS
+    // work counters of the persistent kernels: per call, because one handle may serve several streams
+    unsigned int *counters = nullptr;
+    CK(cudaMallocAsync((void **)&counters, 2 * sizeof(unsigned int), o.stream));
+    struct Free { unsigned int *p; cudaStream_t s; ~Free() { cudaFreeAsync(p, s); } } free_counters{counters, o.stream};
     if (R == 32 && ipls_r32_supported(L)) {
-        unsigned int *counter = nullptr;      // per call: the same handle may serve several streams
-        CK(cudaMallocAsync((void **)&counter, sizeof(unsigned int), o.stream));
-        cudaError_t e = launch_ipls_r32(lv, prm, lib->sm_count, counter, o.stream);
-        cudaFreeAsync(counter, o.stream);
-        CK(e);
+        CK(launch_ipls_r32(lv, prm, lib->sm_count, counters, o.stream));
         ++launches;
     } else if (R <= 64) {
         const int teams = 8, block = teams * 32;
@@ -151,7 +152,10 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     }
     if (lib->timing) CK(cudaEventRecord(lib->ev[1], o.stream));
     // ---- K2: exact finish + uncertainty + residual
-    {
+    if (finish_fast_supported(L, R)) {
+        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 1, o.stream));
+        ++launches;
+    } else {
         const int KMAX = R <= 32 ? R : 64;
         size_t per_warp = (finish_warp_bytes(L, R, KMAX) + 15) & ~(size_t)15;
         int warps = (int)std::min<size_t>(8, (200 * 1024) / per_warp);
