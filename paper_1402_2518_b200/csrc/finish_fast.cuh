@@ -67,8 +67,10 @@ __device__ __forceinline__ float reduce4(float v0, float v1, float v2, float v3,
 
 template <int LV>
 __global__ void __launch_bounds__(512, 1)
-finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter) {
+finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter,
+                   const unsigned int *__restrict__ list /* NULL: all pixels; else [0] = count, [1 + i] = pixel */) {
     using namespace ff;
+    if (list && list[0] == 0u) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int L = lib.L, R = lib.R;
     const int AST = ast(LV);
@@ -101,7 +103,11 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
         unsigned int pu = 0;
         if (lane == 0) pu = atomicAdd(counter, 1u);
         pu = __shfl_sync(FULL, pu, 0);
-        const int64_t p = (int64_t)pu;
+        int64_t p = (int64_t)pu;
+        if (list) {
+            if (pu >= list[0]) break;
+            p = (int64_t)list[1 + pu];
+        }
         if (p >= prm.N) break;
         float *cout = prm.coeffs + p * R;
         int info = prm.info ? prm.info[p] : 0;
@@ -518,7 +524,7 @@ inline int finish_fast_lv(int L) { return L <= 128 ? 1 : (L <= 256 ? 2 : 4); }
 
 template <int LV>
 inline cudaError_t launch_finish_fast_lv(const LibView &lv, const SolveParams &prm, int sm_count,
-                                         unsigned int *counter, cudaStream_t stream) {
+                                         unsigned int *counter, const unsigned int *list, cudaStream_t stream) {
     const size_t cta = (ff::cta_bytes(lv.R, LV) + 15) & ~(size_t)15;
     const size_t per_warp = (ff::warp_bytes(LV) + 15) & ~(size_t)15;
     int warps = (int)std::min<size_t>(16, (220 * 1024 - cta) / per_warp);
@@ -528,18 +534,17 @@ inline cudaError_t launch_finish_fast_lv(const LibView &lv, const SolveParams &p
     if (e != cudaSuccess) return e;
     int64_t need = (prm.N + warps - 1) / warps;
     int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, sm_count));
-    e = cudaMemsetAsync(counter, 0, sizeof(unsigned int), stream);
-    if (e != cudaSuccess) return e;
-    finish_fast_kernel<LV><<<grid, warps * 32, smem, stream>>>(lv, prm, counter);
+    finish_fast_kernel<LV><<<grid, warps * 32, smem, stream>>>(lv, prm, counter, list);
     return cudaGetLastError();
 }
 
+// counter must be zero (the caller clears it on the stream); list: see the kernel
 inline cudaError_t launch_finish_fast(const LibView &lv, const SolveParams &prm, int sm_count,
-                                      unsigned int *counter, cudaStream_t stream) {
+                                      unsigned int *counter, const unsigned int *list, cudaStream_t stream) {
     switch (finish_fast_lv(lv.L)) {
-        case 1: return launch_finish_fast_lv<1>(lv, prm, sm_count, counter, stream);
-        case 2: return launch_finish_fast_lv<2>(lv, prm, sm_count, counter, stream);
-        default: return launch_finish_fast_lv<4>(lv, prm, sm_count, counter, stream);
+        case 1: return launch_finish_fast_lv<1>(lv, prm, sm_count, counter, list, stream);
+        case 2: return launch_finish_fast_lv<2>(lv, prm, sm_count, counter, list, stream);
+        default: return launch_finish_fast_lv<4>(lv, prm, sm_count, counter, list, stream);
     }
 }
 

@@ -378,7 +378,7 @@ inline bool ipls_r32_supported(int L) {
     return r32::smem_floats(L) * sizeof(float) <= 200 * 1024;
 }
 
-// counter: device word, zeroed here on the stream before the launch
+// counter: device word, zero (the caller clears it on the stream before the launch)
 inline cudaError_t launch_ipls_r32(const LibView &lv, const SolveParams &prm, int sm_count,
                                    unsigned int *counter, cudaStream_t stream) {
     size_t smem = r32::smem_floats(lv.L) * sizeof(float);
@@ -391,8 +391,6 @@ inline cudaError_t launch_ipls_r32(const LibView &lv, const SolveParams &prm, in
     int64_t groups = (prm.N + 3) / 4;
     int64_t need = (groups + r32::WARPS - 1) / r32::WARPS;
     int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, (int64_t)sm_count * occ));
-    e = cudaMemsetAsync(counter, 0, sizeof(unsigned int), stream);
-    if (e != cudaSuccess) return e;
     ipls_r32_kernel<<<grid, r32::WARPS * 32, smem, stream>>>(lv, prm, counter);
     return cudaGetLastError();
 }

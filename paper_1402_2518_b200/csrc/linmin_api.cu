@@ -11,6 +11,7 @@
 
 #include "common.cuh"
 #include "finish.cuh"
+#include "finish8.cuh"
 #include "finish_fast.cuh"
 #include "ipls_generic.cuh"
 #include "ipls_r32.cuh"
@@ -126,10 +127,15 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     if (lib->timing) CK(cudaEventRecord(lib->ev[0], o.stream));
 
     // ---- K1: projection + IPLS
-    // work counters of the persistent kernels: per call, because one handle may serve several streams
-    unsigned int *counters = nullptr;
-    CK(cudaMallocAsync((void **)&counters, 2 * sizeof(unsigned int), o.stream));
-    struct Free { unsigned int *p; cudaStream_t s; ~Free() { cudaFreeAsync(p, s); } } free_counters{counters, o.stream};
+    // per-call workspace, because one handle may serve several streams: three work counters of the
+    // persistent kernels, then the overflow list of finish8 (count + one entry per pixel)
+    const bool use_f8 = finish8_supported(L, R);
+    unsigned int *ws = nullptr;
+    const size_t ws_words = 4 + (use_f8 ? (size_t)N + 1 : 0);
+    CK(cudaMallocAsync((void **)&ws, ws_words * sizeof(unsigned int), o.stream));
+    struct Free { unsigned int *p; cudaStream_t s; ~Free() { cudaFreeAsync(p, s); } } free_ws{ws, o.stream};
+    CK(cudaMemsetAsync(ws, 0, std::min<size_t>(5, ws_words) * sizeof(unsigned int), o.stream));
+    unsigned int *counters = ws, *overflow = ws + 4;
     if (R == 32 && ipls_r32_supported(L)) {
         CK(launch_ipls_r32(lv, prm, lib->sm_count, counters, o.stream));
         ++launches;
@@ -152,8 +158,14 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     }
     if (lib->timing) CK(cudaEventRecord(lib->ev[1], o.stream));
     // ---- K2: exact finish + uncertainty + residual
-    if (finish_fast_supported(L, R)) {
-        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 1, o.stream));
+    if (use_f8) {
+        CK(launch_finish8(lv, prm, lib->sm_count, counters + 1, overflow, o.stream));
+        ++launches;
+        // pixels whose support outgrew finish8 (none on the synthetic cubes): one-warp-per-pixel kernel
+        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, o.stream));
+        ++launches;
+    } else if (finish_fast_supported(L, R)) {
+        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, nullptr, o.stream));
         ++launches;
     } else {
         const int KMAX = R <= 32 ? R : 64;

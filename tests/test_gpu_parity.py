@@ -180,6 +180,29 @@ def test_degenerate_inputs(lm):
     assert e.value.code == lm.ERR_LIBRARY_NONFINITE
 
 
+def test_large_supports_take_the_overflow_path(lm):
+    """Supports beyond finish8's cap (16 members) are finished by the one-warp-per-pixel kernel:
+    dense abundances on a well-conditioned random library, mixed with sparse pixels."""
+    import oracle
+    from parity import check_parity
+    rng = np.random.default_rng(77)
+    L, R, N = 128, 32, 600
+    A = rng.uniform(0.1, 0.9, (L, R)).astype(np.float32)
+    a0 = rng.dirichlet(5.0 * np.ones(R), size=N)
+    sparse = rng.uniform(size=N) < 0.5
+    for p in np.nonzero(sparse)[0]:
+        a0[p] = 0.0
+        kk = rng.integers(1, 6)
+        a0[p, rng.choice(R, kk, replace=False)] = rng.dirichlet(np.ones(kk))
+    sig = rng.uniform(0.0005, 0.002, (N, L)).astype(np.float32)
+    Y = (a0 @ A.astype(np.float64).T + sig * rng.standard_normal((N, L))).astype(np.float32)
+    g = run_gpu(lm, A, Y, sig)
+    ora = oracle.solve(A, Y, sig)
+    ksz = (g["info"] >> 24) & 0xff
+    assert (ksz > 16).sum() > 100 and (ksz <= 16).sum() > 100
+    print(check_parity(A, Y, sig, g, ora, label="overflow"))
+
+
 def test_scale_and_offset_invariance(lm):
     """R13: relative stopping rules -> (cA, cy) gives the same coefficients; offset invariance (eq. 4)."""
     from paper_1402_2518_b200.synth import make_workload
