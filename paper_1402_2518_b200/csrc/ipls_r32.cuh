@@ -1,22 +1,24 @@
-// ipls_r32.cuh -- register-blocked projection + IPLS kernel for R = 32 endmembers (sm_100a).
+// ipls_r32.cuh -- register-blocked projection + IPLS kernel for R = 32 endmembers (sm_100a), v3.
 //
 // Same iteration as ipls_generic.cuh (Mehrotra predictor-corrector on the centred normal equations;
 // PAPER.md:71-73 names IPLS and prints no steps -- DESIGN.md reading R1), mapped to the hardware:
 //
 //   * 8 lanes cooperate on one pixel, 4 pixels per warp.  Lane t of a group owns rows
 //     i = t + 8 s (s = 0..3, cyclic) of the 32 x 32 Newton matrix M = G + diag(lambda/a): row i is
-//     kept in REGISTERS up to column 8 s + 7 (80 registers for the lower triangle plus the
-//     upper part of the diagonal blocks, which is kept at zero).
-//   * Right-looking Cholesky, fully unrolled (static register indices).  Column k of L is broadcast
-//     to the group through a double-buffered, bank-padded shared-memory line (<= 4 STS.32, one
-//     __syncwarp, <= 8 LDS.128 per step): 16 FMAs per LDS.128 instead of 1 per shuffle.
-//   * Forward substitution in broadcast form (one shuffle per row and right-hand side), backward
-//     substitution in reduction form (3-shuffle group sum per row), both on the register-resident L.
-//     The sum-to-one multiplier is eliminated through w = L^-1 1, so an iteration needs three
-//     forward and two backward substitutions.
+//     kept in REGISTERS up to column 8 s + 7, as 40 packed pairs (80 registers), so that the
+//     rank-one updates are FFMA2 (fma.rn.f32x2: two FMAs per issue slot).
+//   * Square-root-free Cholesky M = L D L', right-looking, fully unrolled (static register indices).
+//     Step k: every lane puts its raw entries of column k on a double-buffered, bank-padded shared
+//     line, one __syncwarp, every lane reads the column back with LDS.128 (16 FMAs per load) and forms
+//     1/d_k itself: no shuffle, no square root on the dependent chain of a step.
+//   * The forward substitution of the predictor (right-hand sides 1 and -w) is fused into the
+//     factorisation: the two right-hand sides ride along as a packed pair per row.
+//   * Backward substitutions in broadcast form: after the factorisation each lane writes its rows of
+//     L (xor-swizzled, conflict-free) to a per-pixel shared area; step k is one shuffle (x_k), one
+//     LDS (row k of L at my columns) and <= 4 FMAs -- instead of a 3-shuffle reduction per row.
 //   * G (padded rows), the centred library (re-laid out so that a lane's four rows are one LDS.128)
-//     and the channel means live in shared memory, loaded once per CTA; warps then run independently
-//     and fetch groups of 4 pixels from a global atomic counter (per-pixel iteration counts vary).
+//     and the channel means live in shared memory, loaded once per CTA (one CTA of 12 warps per SM);
+//     warps run independently and fetch groups of 4 pixels from a global atomic counter.
 //
 // Algorithmic work per pixel: 2 L R + it (R^3/3 + 8 R^2 + 30 R) flops.
 #pragma once
@@ -28,8 +30,11 @@ namespace r32 {
 
 constexpr int R = 32;
 constexpr int GST = 36;        // padded row stride of G in shared memory (bank-conflict-free LDS.128)
-constexpr int XST = 40;        // per-pixel stride of the exchange lines (4 pixels -> 4 x 8 banks)
-constexpr int WARPS = 4;       // warps per CTA
+constexpr int XST = 56;        // one exchange line: 32 column entries + 8 x 2 right-hand sides + pad
+constexpr int LRS = 712;       // per-pixel factor-row area (704 used; 712 = 8 mod 32 spreads the pixels)
+constexpr int LR0 = 0, LR1 = 64, LR2 = 192, LR3 = 448;   // rows of slot s: 8 lanes x {1, 2, 4, 4} floats
+constexpr int PIXF = 2 * XST + LRS;   // floats per pixel
+constexpr int WARPS = 12;      // warps per CTA, one CTA per SM
 constexpr unsigned FULL = 0xffffffffu;
 
 __device__ __forceinline__ float rcp_approx(float x) {
@@ -37,6 +42,24 @@ __device__ __forceinline__ float rcp_approx(float x) {
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
+__device__ __forceinline__ unsigned long long pk2(float2 v) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(v.x), "f"(v.y));
+    return r;
+}
+__device__ __forceinline__ float2 upk2(unsigned long long v) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+// packed FMA (sm_100 FFMA2): a * b + c on both halves; the scalar form broadcasts a
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pk2(a)), "l"(pk2(b)), "l"(pk2(c)));
+    return upk2(d);
+}
+__device__ __forceinline__ float2 fma2(float a, float2 b, float2 c) { return fma2(make_float2(a, a), b, c); }
+
 __device__ __forceinline__ float gsum(float v) {   // sum over the 8 lanes of a pixel group
     v += __shfl_xor_sync(FULL, v, 1);
     v += __shfl_xor_sync(FULL, v, 2);
@@ -52,67 +75,71 @@ __device__ __forceinline__ float gmax(float v) {
 
 // shared-memory footprint in floats
 __host__ __device__ inline int lpad(int L) { return (L + 3) & ~3; }
-__host__ __device__ inline int ystride(int L) { return lpad(L) + 8; }
 __host__ __device__ inline size_t smem_floats(int L) {
     return (size_t)R * GST + R                 // Gp, row sums
            + (size_t)lpad(L) * R + lpad(L)      // Acp, c
-           + (size_t)WARPS * (4 * ystride(L) + 2 * 4 * XST);
+           + (size_t)WARPS * 4 * PIXF;
 }
 
-// L z = r for NR right-hand sides (in place; r[q][s] ends as z at row t + 8 s)
-template <int NR>
-__device__ __forceinline__ void forward_subst(const float (&m)[4][32], const float (&dinv)[4],
-                                              float (&r)[NR][4], int t) {
+// column j of the register-resident matrix (static j)
+#define LM_COL(s, j) (((j) & 1) ? m2[s][(j) >> 1].y : m2[s][(j) >> 1].x)
+
+// L z = r for ONE right-hand side, L unit lower, m2 holds -L (zeros on and above the diagonal of the
+// diagonal blocks): broadcast form, one shuffle per row.
+__device__ __forceinline__ void forward_subst1(const float2 (&m2)[4][16], float (&r)[4]) {
 #pragma unroll
-    for (int j = 0; j < 32; ++j) {
+    for (int j = 0; j < 31; ++j) {
         const int s0 = j >> 3, t0 = j & 7;
+        const float zj = __shfl_sync(FULL, r[s0], t0, 8);
 #pragma unroll
-        for (int q = 0; q < NR; ++q) {
-            float z = r[q][s0] * dinv[s0];
-            float zj = __shfl_sync(FULL, z, t0, 8);
-            // rows above j in this slot have m[s0][j] == 0 (upper part kept at zero): unchanged
-            float upd = fmaf(-m[s0][j], zj, r[q][s0]);
-            r[q][s0] = (t == t0) ? zj : upd;
-#pragma unroll
-            for (int s = s0 + 1; s < 4; ++s) r[q][s] = fmaf(-m[s][j], zj, r[q][s]);
-        }
+        for (int s = s0; s < 4; ++s) r[s] = fmaf(LM_COL(s, j), zj, r[s]);
     }
 }
 
-// L' x = z (reduction form); x[s] at row t + 8 s
-__device__ __forceinline__ void backward_subst(const float (&m)[4][32], const float (&dinv)[4],
-                                               const float (&z)[4], float (&x)[4], int t) {
+// L' x = y in place, broadcast form; row k of -L comes from the pixel's shared factor-row area
+__device__ __forceinline__ void backward_subst(const float *__restrict__ Lr, float (&y)[4], int t) {
 #pragma unroll
-    for (int s = 0; s < 4; ++s) x[s] = 0.0f;
-#pragma unroll
-    for (int i = 31; i >= 0; --i) {
-        const int s0 = i >> 3, t0 = i & 7;
-        float part = 0.0f;
-#pragma unroll
-        for (int s = s0; s < 4; ++s) part = fmaf(m[s][i], x[s], part);
-        float tot = gsum(part);
-        float xi = (z[s0] - tot) * dinv[s0];
-        x[s0] = (t == t0) ? xi : x[s0];
+    for (int k = 31; k >= 1; --k) {
+        const int s0 = k >> 3, t0 = k & 7;
+        const float xk = __shfl_sync(FULL, y[s0], t0, 8);
+        const int pos = t ^ t0;
+        if (s0 == 3) {
+            const float4 v = *reinterpret_cast<const float4 *>(Lr + LR3 + t0 * 32 + 4 * pos);
+            y[0] = fmaf(v.x, xk, y[0]); y[1] = fmaf(v.y, xk, y[1]); y[2] = fmaf(v.z, xk, y[2]);
+            if (t0 > 0) y[3] = fmaf(v.w, xk, y[3]);
+        } else if (s0 == 2) {
+            const float4 v = *reinterpret_cast<const float4 *>(Lr + LR2 + t0 * 32 + 4 * pos);
+            y[0] = fmaf(v.x, xk, y[0]); y[1] = fmaf(v.y, xk, y[1]);
+            if (t0 > 0) y[2] = fmaf(v.z, xk, y[2]);
+        } else if (s0 == 1) {
+            const float2 v = *reinterpret_cast<const float2 *>(Lr + LR1 + t0 * 16 + 2 * pos);
+            y[0] = fmaf(v.x, xk, y[0]);
+            if (t0 > 0) y[1] = fmaf(v.y, xk, y[1]);
+        } else {
+            const float v = Lr[LR0 + t0 * 8 + pos];
+            y[0] = fmaf(v, xk, y[0]);
+        }
     }
 }
 
 }  // namespace r32
 
-__global__ void __launch_bounds__(r32::WARPS * 32, 3)
+__global__ void __launch_bounds__(r32::WARPS * 32, 1)
 ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter) {
     using namespace r32;
     extern __shared__ __align__(16) float smem[];
     const int L = lib.L;
-    const int Lp = lpad(L), YST = ystride(L);
+    const int Lp = lpad(L);
     float *Gp = smem;                        // [32][GST]
     float *Grs = Gp + R * GST;               // [32] row sums of G
     float *Acp = Grs + R;                    // [Lp][32]: Acp[l][t*4+s] = Ac[l][t+8s]
     float *cv = Acp + (size_t)Lp * R;        // [Lp]
-    float *wbase = cv + Lp + (size_t)(threadIdx.x >> 5) * (4 * YST + 2 * 4 * XST);
     const int lane = threadIdx.x & 31, g = lane >> 3, t = lane & 7;
-    float *ybuf = wbase + g * YST;                         // this pixel's centred spectrum
-    float *xb0 = wbase + 4 * YST + g * XST;                // exchange line, buffer 0
-    float *xb1 = xb0 + 4 * XST;                            // buffer 1
+    float *pix = cv + Lp + (size_t)((threadIdx.x >> 5) * 4 + g) * PIXF;
+    float *xb0 = pix;                        // exchange line, buffer 0
+    float *xb1 = pix + XST;                  // buffer 1
+    float *Lr = pix + 2 * XST;               // factor rows (backward substitution)
+    float *ybuf = Lr;                        // the centred spectrum lives here during the projection only
 
     // ---- once per CTA: stage the library data
     for (int e = threadIdx.x; e < R * R; e += blockDim.x) Gp[(e >> 5) * GST + (e & 31)] = lib.Gc[e];
@@ -132,6 +159,10 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
     const float gdmax = lib.gdmax;
     const float tau = 0.995f;
     const float pivot_floor = 1e-12f * gdmax;
+    // one-hot pairs of my position inside a diagonal block: adds lambda/a to the diagonal with FFMA2
+    float2 e2[4];
+#pragma unroll
+    for (int jp = 0; jp < 4; ++jp) e2[jp] = make_float2((t == 2 * jp) ? 1.0f : 0.0f, (t == 2 * jp + 1) ? 1.0f : 0.0f);
 
     while (true) {
         unsigned int grp = 0;
@@ -145,6 +176,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         // ---- load the spectrum (8 lanes x 4 B = one 32 B sector per step), centre, flag non-finite
         const float *y = prm.Y + p * prm.ldY;
         bool bad = false;
+        __syncwarp();
         for (int l = t; l < Lp; l += 8) {
             float yv = (l < L) ? y[l] : 0.0f;
             bad |= !isfinite(yv);
@@ -156,18 +188,19 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         __syncwarp();
 
         // ---- projection b = Ac'(y - c)
-        float b[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+        float2 b01 = make_float2(0.0f, 0.0f), b23 = make_float2(0.0f, 0.0f);
         for (int l4 = 0; l4 < Lp; l4 += 4) {
-            float4 y4 = *reinterpret_cast<const float4 *>(ybuf + l4);
-            float4 a0 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 0) * R + t * 4);
-            float4 a1 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 1) * R + t * 4);
-            float4 a2 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 2) * R + t * 4);
-            float4 a3 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 3) * R + t * 4);
-            b[0] = fmaf(a0.x, y4.x, b[0]); b[1] = fmaf(a0.y, y4.x, b[1]); b[2] = fmaf(a0.z, y4.x, b[2]); b[3] = fmaf(a0.w, y4.x, b[3]);
-            b[0] = fmaf(a1.x, y4.y, b[0]); b[1] = fmaf(a1.y, y4.y, b[1]); b[2] = fmaf(a1.z, y4.y, b[2]); b[3] = fmaf(a1.w, y4.y, b[3]);
-            b[0] = fmaf(a2.x, y4.z, b[0]); b[1] = fmaf(a2.y, y4.z, b[1]); b[2] = fmaf(a2.z, y4.z, b[2]); b[3] = fmaf(a2.w, y4.z, b[3]);
-            b[0] = fmaf(a3.x, y4.w, b[0]); b[1] = fmaf(a3.y, y4.w, b[1]); b[2] = fmaf(a3.z, y4.w, b[2]); b[3] = fmaf(a3.w, y4.w, b[3]);
+            const float4 y4 = *reinterpret_cast<const float4 *>(ybuf + l4);
+            const float4 a0 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 0) * R + t * 4);
+            const float4 a1 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 1) * R + t * 4);
+            const float4 a2 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 2) * R + t * 4);
+            const float4 a3 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 3) * R + t * 4);
+            b01 = fma2(y4.x, make_float2(a0.x, a0.y), b01); b23 = fma2(y4.x, make_float2(a0.z, a0.w), b23);
+            b01 = fma2(y4.y, make_float2(a1.x, a1.y), b01); b23 = fma2(y4.y, make_float2(a1.z, a1.w), b23);
+            b01 = fma2(y4.z, make_float2(a2.x, a2.y), b01); b23 = fma2(y4.z, make_float2(a2.z, a2.w), b23);
+            b01 = fma2(y4.w, make_float2(a3.x, a3.y), b01); b23 = fma2(y4.w, make_float2(a3.z, a3.w), b23);
         }
+        const float b[4] = {b01.x, b01.y, b23.x, b23.y};
         float bmax = gmax(fmaxf(fmaxf(fabsf(b[0]), fabsf(b[1])), fmaxf(fabsf(b[2]), fabsf(b[3]))));
         const float sc = fmaxf(bmax, 1e-3f * gdmax);
 
@@ -187,25 +220,26 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         bool done = false;
 
         for (int it = 0;; ++it) {
-            // ---- exchange a; G a and the Newton matrix rows from shared memory
-            float *xe = (it & 1) ? xb1 : xb0;      // this iteration's "even" line
-            float *xo = (it & 1) ? xb0 : xb1;
+            // ---- exchange a (line 1: step 0 of the factorisation writes line 0); G a and M rows
             __syncwarp();
 #pragma unroll
-            for (int s = 0; s < 4; ++s) xe[t + 8 * s] = a[s];
+            for (int s = 0; s < 4; ++s) xb1[t + 8 * s] = a[s];
             __syncwarp();
-            float m[4][32];
-            float Ga[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+            float2 m2[4][16];
+            float2 Ga2[4];
+#pragma unroll
+            for (int s = 0; s < 4; ++s) Ga2[s] = make_float2(0.0f, 0.0f);
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
-                float4 a4 = *reinterpret_cast<const float4 *>(xe + 4 * c);
+                const float4 a4 = *reinterpret_cast<const float4 *>(xb1 + 4 * c);
 #pragma unroll
                 for (int s = 0; s < 4; ++s) {
-                    float4 g4 = *reinterpret_cast<const float4 *>(Gp + (t + 8 * s) * GST + 4 * c);
-                    Ga[s] = fmaf(g4.x, a4.x, Ga[s]); Ga[s] = fmaf(g4.y, a4.y, Ga[s]);
-                    Ga[s] = fmaf(g4.z, a4.z, Ga[s]); Ga[s] = fmaf(g4.w, a4.w, Ga[s]);
+                    const float4 g4 = *reinterpret_cast<const float4 *>(Gp + (t + 8 * s) * GST + 4 * c);
+                    Ga2[s] = fma2(make_float2(g4.x, g4.y), make_float2(a4.x, a4.y), Ga2[s]);
+                    Ga2[s] = fma2(make_float2(g4.z, g4.w), make_float2(a4.z, a4.w), Ga2[s]);
                     if (4 * c < 8 * s + 8) {
-                        m[s][4 * c + 0] = g4.x; m[s][4 * c + 1] = g4.y; m[s][4 * c + 2] = g4.z; m[s][4 * c + 3] = g4.w;
+                        m2[s][2 * c] = make_float2(g4.x, g4.y);
+                        m2[s][2 * c + 1] = make_float2(g4.z, g4.w);
                     }
                 }
             }
@@ -213,7 +247,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             float rdm = 0.0f, sa = 0.0f, gp = 0.0f;
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
-                w[s] = Ga[s] - b[s] + nu;
+                w[s] = Ga2[s].x + Ga2[s].y - b[s] + nu;
                 rdm = fmaxf(rdm, fabsf(w[s] - lam[s]));
                 sa += a[s];
                 gp = fmaf(a[s], lam[s], gp);
@@ -231,7 +265,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             if (!done) ++iters;
             const float mu = gp * (1.0f / 32.0f);
 
-            // ---- M = G + diag(lambda / a); upper part of the diagonal blocks := 0
+            // ---- M = G + diag(lambda / a)
             float ainv[4], d[4], dinv[4];
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
@@ -239,76 +273,97 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                 d[s] = lam[s] * ainv[s];
                 dinv[s] = 0.0f;
 #pragma unroll
-                for (int jj = 0; jj < 8; ++jj) {
-                    float v = m[s][8 * s + jj];
-                    v = (jj == t) ? v + d[s] : v;
-                    m[s][8 * s + jj] = (jj <= t) ? v : 0.0f;
-                }
+                for (int jp = 0; jp < 4; ++jp) m2[s][4 * s + jp] = fma2(d[s], e2[jp], m2[s][4 * s + jp]);
             }
-            // ---- Cholesky, right-looking, column broadcast through shared memory
+            // ---- M = L D L' (right-looking), with the predictor's forward substitution riding along:
+            //      rr[s] = (row of L^-1 1, row of L^-1 (-w)).  m2 ends as -L (strictly lower; zeros on and
+            //      above the diagonal inside the diagonal blocks), dinv = 1 / d.
+            float2 rr[4];
+#pragma unroll
+            for (int s = 0; s < 4; ++s) rr[s] = make_float2(1.0f, -w[s]);
             bool clamped = false;
 #pragma unroll
-            for (int k = 0; k < 32; ++k) {
+            for (int k = 0; k < 31; ++k) {
                 const int s0 = k >> 3, t0 = k & 7;
-                float *cb = (k & 1) ? xe : xo;       // alternate lines: no WAR hazard with one sync per step
-                float piv = __shfl_sync(FULL, m[s0][k], t0, 8);
+                float *cb = (k & 1) ? xb1 : xb0;       // alternate lines: one sync per step is enough
+#pragma unroll
+                for (int s = s0; s < 4; ++s) cb[t + 8 * s] = LM_COL(s, k);
+                *reinterpret_cast<float2 *>(cb + 32 + 2 * t) = rr[s0];
+                __syncwarp();
+                const float2 zk = *reinterpret_cast<const float2 *>(cb + 32 + 2 * t0);
+                // column chunks from the one that holds k + 1; the pivot sits in chunk k >> 2
+                float4 l4[8];
+#pragma unroll
+                for (int c = (k + 1) >> 2; c < 8; ++c) l4[c] = *reinterpret_cast<const float4 *>(cb + 4 * c);
+                float piv;
+                if (((k + 1) & 3) == 0) piv = cb[k];
+                else piv = ((k & 3) == 0) ? l4[k >> 2].x : (((k & 3) == 1) ? l4[k >> 2].y : l4[k >> 2].z);
                 if (!(piv > pivot_floor)) { piv = pivot_floor; clamped = true; }
-                float rinv = rsqrtf(piv);
-                float lcol[4];
+                const float rinv = rcp_approx(piv);
+                const float nrinv = -rinv;
+                float nl[4];
 #pragma unroll
                 for (int s = s0; s < 4; ++s) {
-                    // slot s0: rows above k hold 0 (stay 0), row k itself becomes L_kk
-                    lcol[s] = m[s][k] * rinv;
-                    m[s][k] = lcol[s];
-                    cb[t + 8 * s] = lcol[s];
+                    float v = LM_COL(s, k) * nrinv;
+                    if (s == s0) v = (t > t0) ? v : 0.0f;      // rows at or above k: no update, store 0
+                    nl[s] = v;
+                    if (k & 1) m2[s][k >> 1].y = v; else m2[s][k >> 1].x = v;
+                    rr[s] = fma2(v, zk, rr[s]);
                 }
                 dinv[s0] = (t == t0) ? rinv : dinv[s0];
-                if (k == 31) break;
-                __syncwarp();
-                // rows of slot s0 at or above k must not be touched by the update
-                float lrow0 = (t > t0) ? lcol[s0] : 0.0f;
 #pragma unroll
                 for (int c = (k + 1) >> 2; c < 8; ++c) {
-                    float4 l4 = *reinterpret_cast<const float4 *>(cb + 4 * c);
-                    const float lj[4] = {l4.x, l4.y, l4.z, l4.w};
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const int j = 4 * c + q;
-                        if (j > k) {
+                    for (int h = 0; h < 2; ++h) {
+                        const int jp = 2 * c + h, j0 = 2 * jp;
+                        const float2 cp = h ? make_float2(l4[c].z, l4[c].w) : make_float2(l4[c].x, l4[c].y);
+                        if (j0 > k) {
 #pragma unroll
-                            for (int s = s0; s < 4; ++s) {
-                                if (j < 8 * s + 8) {
-                                    float li = (s == s0) ? lrow0 : lcol[s];
-                                    m[s][j] = fmaf(-li, lj[q], m[s][j]);
-                                }
-                            }
+                            for (int s = s0; s < 4; ++s)
+                                if (j0 < 8 * s + 8) m2[s][jp] = fma2(nl[s], cp, m2[s][jp]);
+                        } else if (j0 == k) {
+#pragma unroll
+                            for (int s = s0; s < 4; ++s)
+                                if (j0 < 8 * s + 8) m2[s][jp].y = fmaf(nl[s], cp.y, m2[s][jp].y);
                         }
                     }
                 }
             }
-            if (clamped) flags |= LINMIN_INFO_CHOL_REGULARISED;
-            // the in-block upper entries were updated with li = 0 only for rows <= k of slot s0 at
-            // step k; entries (i, j), j > i, of LATER steps k < i still received updates: clear them
+            {   // k = 31: only the last pivot (its owner has it) -- nothing left to update
+                float piv = m2[3][15].y;
+                if (t == 7 && !(piv > pivot_floor)) { piv = pivot_floor; clamped = true; }
+                dinv[3] = (t == 7) ? rcp_approx(piv) : dinv[3];
+                m2[3][15].y = 0.0f;
+            }
+            if (__any_sync(0xffu << (8 * g), clamped)) flags |= LINMIN_INFO_CHOL_REGULARISED;
+            // ---- rows of -L to the shared factor-row area (chunk of reader lane t' at position t' ^ t)
 #pragma unroll
-            for (int s = 0; s < 4; ++s)
-#pragma unroll
-                for (int jj = 1; jj < 8; ++jj) m[s][8 * s + jj] = (jj <= t) ? m[s][8 * s + jj] : 0.0f;
+            for (int tp = 0; tp < 8; ++tp) {
+                const int pos = tp ^ t;
+                Lr[LR0 + t * 8 + pos] = LM_COL(0, tp);
+                *reinterpret_cast<float2 *>(Lr + LR1 + t * 16 + 2 * pos) = make_float2(LM_COL(1, tp), LM_COL(1, 8 + tp));
+                *reinterpret_cast<float4 *>(Lr + LR2 + t * 32 + 4 * pos) =
+                    make_float4(LM_COL(2, tp), LM_COL(2, 8 + tp), LM_COL(2, 16 + tp), 0.0f);
+                *reinterpret_cast<float4 *>(Lr + LR3 + t * 32 + 4 * pos) =
+                    make_float4(LM_COL(3, tp), LM_COL(3, 8 + tp), LM_COL(3, 16 + tp), LM_COL(3, 24 + tp));
+            }
+            __syncwarp();
 
-            // ---- predictor: w1 = L^-1 1, z = L^-1 (-w)
-            float r2[2][4];
-#pragma unroll
-            for (int s = 0; s < 4; ++s) { r2[0][s] = 1.0f; r2[1][s] = -w[s]; }
-            forward_subst<2>(m, dinv, r2, t);
+            // ---- predictor: M^-1 = L^-T D^-1 L^-1; nu eliminated through L^-1 1
             float sww = 0.0f, swz = 0.0f;
 #pragma unroll
-            for (int s = 0; s < 4; ++s) { sww = fmaf(r2[0][s], r2[0][s], sww); swz = fmaf(r2[0][s], r2[1][s], swz); }
+            for (int s = 0; s < 4; ++s) {
+                const float zd = rr[s].x * dinv[s];
+                sww = fmaf(zd, rr[s].x, sww);
+                swz = fmaf(zd, rr[s].y, swz);
+            }
             sww = gsum(sww); swz = gsum(swz);
             const float rsww = 1.0f / sww;
             float dnu = (swz + rp) * rsww;
-            float zz[4], da[4], dl[4];
+            float da[4], dl[4];
 #pragma unroll
-            for (int s = 0; s < 4; ++s) zz[s] = fmaf(-r2[0][s], dnu, r2[1][s]);
-            backward_subst(m, dinv, zz, da, t);
+            for (int s = 0; s < 4; ++s) da[s] = fmaf(-rr[s].x, dnu, rr[s].y) * dinv[s];
+            backward_subst(Lr, da, t);
             float mp = 0.0f, md = 0.0f;     // max of -da/a and -dl/lambda
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
@@ -326,21 +381,21 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             float sg = mua / mu;
             sg = fminf(1.0f, fmaxf(0.0f, sg * sg * sg));
             // ---- corrector
-            float cc[4], r1[1][4];
+            float cc[4], r1[4];
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
                 cc[s] = fmaf(sg, mu, -da[s] * dl[s]);
-                r1[0][s] = fmaf(cc[s], ainv[s], -w[s]);
+                r1[s] = fmaf(cc[s], ainv[s], -w[s]);
             }
-            forward_subst<1>(m, dinv, r1, t);
+            forward_subst1(m2, r1);
             swz = 0.0f;
 #pragma unroll
-            for (int s = 0; s < 4; ++s) swz = fmaf(r2[0][s], r1[0][s], swz);
+            for (int s = 0; s < 4; ++s) swz = fmaf(rr[s].x * dinv[s], r1[s], swz);
             swz = gsum(swz);
             dnu = (swz + rp) * rsww;
 #pragma unroll
-            for (int s = 0; s < 4; ++s) zz[s] = fmaf(-r2[0][s], dnu, r1[0][s]);
-            backward_subst(m, dinv, zz, da, t);
+            for (int s = 0; s < 4; ++s) da[s] = fmaf(-rr[s].x, dnu, r1[s]) * dinv[s];
+            backward_subst(Lr, da, t);
             mp = 0.0f; md = 0.0f;
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
@@ -373,9 +428,10 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         __syncwarp();
     }
 }
+#undef LM_COL
 
 inline bool ipls_r32_supported(int L) {
-    return r32::smem_floats(L) * sizeof(float) <= 200 * 1024;
+    return r32::lpad(L) <= r32::LRS && r32::smem_floats(L) * sizeof(float) <= 226 * 1024;
 }
 
 // counter: device word, zero (the caller clears it on the stream before the launch)
@@ -384,13 +440,9 @@ inline cudaError_t launch_ipls_r32(const LibView &lv, const SolveParams &prm, in
     size_t smem = r32::smem_floats(lv.L) * sizeof(float);
     cudaError_t e = cudaFuncSetAttribute(ipls_r32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    int occ = 1;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ipls_r32_kernel, r32::WARPS * 32, smem);
-    if (e != cudaSuccess) return e;
-    if (occ < 1) occ = 1;
     int64_t groups = (prm.N + 3) / 4;
     int64_t need = (groups + r32::WARPS - 1) / r32::WARPS;
-    int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, (int64_t)sm_count * occ));
+    int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, (int64_t)sm_count));
     ipls_r32_kernel<<<grid, r32::WARPS * 32, smem, stream>>>(lv, prm, counter);
     return cudaGetLastError();
 }
