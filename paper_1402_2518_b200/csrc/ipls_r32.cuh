@@ -26,6 +26,17 @@
 
 namespace linmin {
 
+#ifdef IPLS_PHASE_PROF
+__device__ unsigned long long g_phase[16];
+#define PH_DECL long long ph_t = clock64(); long long ph_acc[10] = {0,0,0,0,0,0,0,0,0,0};
+#define PH(i) { long long n__ = clock64(); ph_acc[i] += n__ - ph_t; ph_t = n__; }
+#define PH_FLUSH if (lane == 0) { for (int i__ = 0; i__ < 10; ++i__) atomicAdd(&g_phase[i__], (unsigned long long)ph_acc[i__]); }
+#else
+#define PH_DECL
+#define PH(i)
+#define PH_FLUSH
+#endif
+
 namespace r32 {
 
 constexpr int R = 32;
@@ -34,7 +45,7 @@ constexpr int XST = 56;        // one exchange line: 32 column entries + 8 x 2 r
 constexpr int LRS = 712;       // per-pixel factor-row area (704 used; 712 = 8 mod 32 spreads the pixels)
 constexpr int LR0 = 0, LR1 = 64, LR2 = 192, LR3 = 448;   // rows of slot s: 8 lanes x {1, 2, 4, 4} floats
 constexpr int PIXF = 2 * XST + LRS;   // floats per pixel
-constexpr int WARPS = 12;      // warps per CTA, one CTA per SM
+constexpr int WARPS = 8;      // warps per CTA, one CTA per SM
 constexpr unsigned FULL = 0xffffffffu;
 
 __device__ __forceinline__ float rcp_approx(float x) {
@@ -164,7 +175,9 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
 #pragma unroll
     for (int jp = 0; jp < 4; ++jp) e2[jp] = make_float2((t == 2 * jp) ? 1.0f : 0.0f, (t == 2 * jp + 1) ? 1.0f : 0.0f);
 
+    PH_DECL
     while (true) {
+        PH(8)
         unsigned int grp = 0;
         if (lane == 0) grp = atomicAdd(counter, 1u);
         grp = __shfl_sync(FULL, grp, 0);
@@ -219,6 +232,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         int iters = 0, flags = bad ? LINMIN_INFO_NONFINITE_INPUT : 0;
         bool done = false;
 
+        PH(7)
         for (int it = 0;; ++it) {
             // ---- exchange a (line 1: step 0 of the factorisation writes line 0); G a and M rows
             __syncwarp();
@@ -243,6 +257,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                     }
                 }
             }
+            PH(0)
             // ---- residuals and stopping rule (per pixel group)
             float rdm = 0.0f, sa = 0.0f, gp = 0.0f;
 #pragma unroll
@@ -265,6 +280,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             if (!done) ++iters;
             const float mu = gp * (1.0f / 32.0f);
 
+            PH(1)
             // ---- M = G + diag(lambda / a)
             float ainv[4], d[4], dinv[4];
 #pragma unroll
@@ -282,22 +298,26 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
 #pragma unroll
             for (int s = 0; s < 4; ++s) rr[s] = make_float2(1.0f, -w[s]);
             bool clamped = false;
+            // Look-ahead schedule: column k + 1 is updated and put on the exchange line BEFORE the rest of
+            // the rank-one update of step k, so that the shared-memory round trip of step k + 1 overlaps
+            // the FFMA2 stream of step k.  l4[c] / zk hold column k (raw) and the row-k right-hand sides.
+            float4 l4[8];
+            float2 zk;
+            {
+#pragma unroll
+                for (int s = 0; s < 4; ++s) xb0[t + 8 * s] = LM_COL(s, 0);
+                *reinterpret_cast<float2 *>(xb0 + 32 + 2 * t) = rr[0];
+                __syncwarp();
+                zk = *reinterpret_cast<const float2 *>(xb0 + 32);
+#pragma unroll
+                for (int c = 0; c < 8; ++c) l4[c] = *reinterpret_cast<const float4 *>(xb0 + 4 * c);
+            }
+#define L4C(j) ((((j) & 3) == 0) ? l4[(j) >> 2].x : ((((j) & 3) == 1) ? l4[(j) >> 2].y : ((((j) & 3) == 2) ? l4[(j) >> 2].z : l4[(j) >> 2].w)))
 #pragma unroll
             for (int k = 0; k < 31; ++k) {
                 const int s0 = k >> 3, t0 = k & 7;
-                float *cb = (k & 1) ? xb1 : xb0;       // alternate lines: one sync per step is enough
-#pragma unroll
-                for (int s = s0; s < 4; ++s) cb[t + 8 * s] = LM_COL(s, k);
-                *reinterpret_cast<float2 *>(cb + 32 + 2 * t) = rr[s0];
-                __syncwarp();
-                const float2 zk = *reinterpret_cast<const float2 *>(cb + 32 + 2 * t0);
-                // column chunks from the one that holds k + 1; the pivot sits in chunk k >> 2
-                float4 l4[8];
-#pragma unroll
-                for (int c = (k + 1) >> 2; c < 8; ++c) l4[c] = *reinterpret_cast<const float4 *>(cb + 4 * c);
-                float piv;
-                if (((k + 1) & 3) == 0) piv = cb[k];
-                else piv = ((k & 3) == 0) ? l4[k >> 2].x : (((k & 3) == 1) ? l4[k >> 2].y : l4[k >> 2].z);
+                const int k1 = k + 1, s1 = k1 >> 3;
+                float piv = L4C(k);
                 if (!(piv > pivot_floor)) { piv = pivot_floor; clamped = true; }
                 const float rinv = rcp_approx(piv);
                 const float nrinv = -rinv;
@@ -311,24 +331,53 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                     rr[s] = fma2(v, zk, rr[s]);
                 }
                 dinv[s0] = (t == t0) ? rinv : dinv[s0];
+                // ---- look-ahead: column k + 1 first, then its exchange
+                {
+                    const float ck1 = L4C(k1);
 #pragma unroll
-                for (int c = (k + 1) >> 2; c < 8; ++c) {
+                    for (int s = s1; s < 4; ++s) {
+                        if (k1 & 1) m2[s][k1 >> 1].y = fmaf(nl[s], ck1, m2[s][k1 >> 1].y);
+                        else m2[s][k1 >> 1].x = fmaf(nl[s], ck1, m2[s][k1 >> 1].x);
+                    }
+                }
+                float4 n4[8];
+                float2 zn = make_float2(0.0f, 0.0f);
+                if (k1 < 31) {
+                    float *cb = (k1 & 1) ? xb1 : xb0;
+#pragma unroll
+                    for (int s = s1; s < 4; ++s) cb[t + 8 * s] = LM_COL(s, k1);
+                    *reinterpret_cast<float2 *>(cb + 32 + 2 * t) = rr[s1];
+                    __syncwarp();
+                    zn = *reinterpret_cast<const float2 *>(cb + 32 + 2 * (k1 & 7));
+#pragma unroll
+                    for (int c = k1 >> 2; c < 8; ++c) n4[c] = *reinterpret_cast<const float4 *>(cb + 4 * c);
+                }
+                // ---- rest of the rank-one update of step k: columns k + 2 ..
+#pragma unroll
+                for (int c = (k + 2) >> 2; c < 8; ++c) {
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         const int jp = 2 * c + h, j0 = 2 * jp;
                         const float2 cp = h ? make_float2(l4[c].z, l4[c].w) : make_float2(l4[c].x, l4[c].y);
-                        if (j0 > k) {
+                        if (j0 >= k + 2) {
 #pragma unroll
                             for (int s = s0; s < 4; ++s)
                                 if (j0 < 8 * s + 8) m2[s][jp] = fma2(nl[s], cp, m2[s][jp]);
-                        } else if (j0 == k) {
+                        } else if (j0 + 1 == k + 2) {
 #pragma unroll
                             for (int s = s0; s < 4; ++s)
                                 if (j0 < 8 * s + 8) m2[s][jp].y = fmaf(nl[s], cp.y, m2[s][jp].y);
                         }
                     }
                 }
+                if (k1 < 31) {
+                    zk = zn;
+#pragma unroll
+                    for (int c = k1 >> 2; c < 8; ++c) l4[c] = n4[c];
+                }
             }
+#undef L4C
+            PH(2)
             {   // k = 31: only the last pivot (its owner has it) -- nothing left to update
                 float piv = m2[3][15].y;
                 if (t == 7 && !(piv > pivot_floor)) { piv = pivot_floor; clamped = true; }
@@ -349,6 +398,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             }
             __syncwarp();
 
+            PH(3)
             // ---- predictor: M^-1 = L^-T D^-1 L^-1; nu eliminated through L^-1 1
             float sww = 0.0f, swz = 0.0f;
 #pragma unroll
@@ -380,6 +430,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             mua = gsum(mua) * (1.0f / 32.0f);
             float sg = mua / mu;
             sg = fminf(1.0f, fmaxf(0.0f, sg * sg * sg));
+            PH(4)
             // ---- corrector
             float cc[4], r1[4];
 #pragma unroll
@@ -388,6 +439,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                 r1[s] = fmaf(cc[s], ainv[s], -w[s]);
             }
             forward_subst1(m2, r1);
+            PH(5)
             swz = 0.0f;
 #pragma unroll
             for (int s = 0; s < 4; ++s) swz = fmaf(rr[s].x * dinv[s], r1[s], swz);
@@ -413,6 +465,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                 lam[s] = fmaxf(fmaf(ad, dl[s], lam[s]), 1e-18f * lam0);
             }
             nu = fmaf(ad, dnu, nu);
+            PH(6)
         }
 
         // ---- store the iterate (coalesced: 8 lanes x float4 = one 128 B row) and the info word
@@ -427,6 +480,8 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         }
         __syncwarp();
     }
+    PH(8)
+    PH_FLUSH
 }
 #undef LM_COL
 

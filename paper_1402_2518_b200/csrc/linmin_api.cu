@@ -13,6 +13,7 @@
 #include "finish.cuh"
 #include "finish8.cuh"
 #include "finish_fast.cuh"
+#include "finish_sweep.cuh"
 #include "ipls_generic.cuh"
 #include "ipls_r32.cuh"
 #include "precompute.cuh"
@@ -159,7 +160,7 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     if (lib->timing) CK(cudaEventRecord(lib->ev[1], o.stream));
     // ---- K2: exact finish + uncertainty + residual
     if (use_f8) {
-        CK(launch_finish8(lv, prm, lib->sm_count, counters + 1, overflow, o.stream));
+        CK(launch_finish_sweep(lv, prm, lib->sm_count, counters + 1, overflow, o.stream));
         ++launches;
         // pixels whose support outgrew finish8 (none on the synthetic cubes): one-warp-per-pixel kernel
         CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, o.stream));
@@ -243,6 +244,14 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
 }  // namespace
 
 extern "C" {
+
+#ifdef IPLS_PHASE_PROF
+int linmin_debug_phases(unsigned long long *out16, int reset) {
+    if (out16) cudaMemcpyFromSymbol(out16, linmin::g_phase, 16 * sizeof(unsigned long long));
+    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(linmin::g_phase, z, sizeof(z)); }
+    return 0;
+}
+#endif
 
 int linmin_version(void) { return LINMIN_VERSION; }
 
