@@ -25,12 +25,13 @@ constexpr unsigned FULL = 0xffffffffu;
 constexpr int KM = 16;    // support cap of this kernel
 constexpr int RP = 32;    // endmember rows staged (rows >= R are zero)
 constexpr int GS = 33;    // row stride of the staged fp64 Gram matrix (bank spread)
+constexpr int MS = 18;    // row stride (doubles) of the per-pixel matrix: 144 B rows, conflict-free LDS.128 by row
 
 // per-pixel scratch (bytes; every block 16 B aligned)
-constexpr int OFF_M = 0;                      // double[16][16], pair chunk c2 of row i at chunk c2 ^ (i & 7)
+constexpr int OFF_M = 0;                      // double[16][MS]
 constexpr int OFF_HS = 0;                     //   later: float[16][16] H (first KB of M)
 constexpr int OFF_EX = 1024;                  //   later: float[8][32] partial sums of A'r (second KB of M)
-constexpr int OFF_BE = 2048;                  // double[32] b_i = A_i'y by endmember
+constexpr int OFF_BE = 16 * MS * 8;           // double[32] b_i = A_i'y by endmember
 constexpr int OFF_BR = OFF_BE + 32 * 8;       // double[16] b by rank
 constexpr int OFF_AF = OFF_BR + 16 * 8;       // double[16] current point by rank
 constexpr int OFF_QV = OFF_AF + 16 * 8;       // double[16] q = K 1 by rank
@@ -38,7 +39,7 @@ constexpr int OFF_G = OFF_QV + 16 * 8;        // float[32] gradient / output sta
 constexpr int OFF_SG = OFF_G + 32 * 4;        // float[16] coeff_sigma by rank
 constexpr int OFF_IDX = OFF_SG + 16 * 4;      // int[16]
 constexpr int OFF_STATE = OFF_IDX + 16 * 4;   // uchar[32]: 0 free, 1 in F, 2 blocked
-constexpr int PIX_BYTES = OFF_STATE + 32;     // 2976
+constexpr int PIX_BYTES = OFF_STATE + 32;     // 3232
 static_assert(PIX_BYTES % 16 == 0, "scratch alignment");
 
 __host__ __device__ inline size_t cta_bytes(int LQ) {
@@ -136,7 +137,7 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) {
 
 // LQ = float4 chunks of the spectrum per lane: L <= 32 LQ
 template <int LQ>
-__global__ void __launch_bounds__(512, 1)
+__global__ void __maxnreg__(144)
 finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter,
                     unsigned int *__restrict__ overflow /* [0] = count, [1 + i] = pixel */) {
     using namespace fs;
@@ -182,8 +183,8 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
     const bool csvec_ok = ((R & 3) == 0) && ((reinterpret_cast<uintptr_t>(prm.coeff_sigma) & 15) == 0);
     const float qnan = __int_as_float(0x7fc00000);
     const int max_pivots = 4 * RP + 8;
-    double *M0 = Md + t * 16;          // my rows of the swept matrix
-    double *M1 = Md + (t + 8) * 16;
+    double *M0 = Md + t * MS;          // my rows of the swept matrix
+    double *M1 = Md + (t + 8) * MS;
 
     while (true) {
         unsigned int grp = 0;
@@ -350,11 +351,11 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                         double2 m0, m1;
                         m0.x = (v0 && t < k) ? G64s[i0 * GS + jj.x] : 0.0;
                         m0.y = (v1 && t < k) ? G64s[i0 * GS + jj.y] : 0.0;
-                        *reinterpret_cast<double2 *>(M0 + 2 * (c2 ^ t)) = m0;
+                        *reinterpret_cast<double2 *>(M0 + 2 * c2) = m0;
                         if (wide) {
                             m1.x = (v0 && t + 8 < k) ? G64s[i1 * GS + jj.x] : 0.0;
                             m1.y = (v1 && t + 8 < k) ? G64s[i1 * GS + jj.y] : 0.0;
-                            *reinterpret_cast<double2 *>(M1 + 2 * (c2 ^ t)) = m1;
+                            *reinterpret_cast<double2 *>(M1 + 2 * c2) = m1;
                         }
                     }
                 }
@@ -364,42 +365,40 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             int rej = -1;
             for (int j = 0; j < kw; ++j) {
                 const bool on = act && rej < 0 && j < k;
-                const int sj = j & 7;
-                const double *Mj = Md + j * 16;
+                const double *Mj = Md + j * MS;
                 double2 rj[8];
 #pragma unroll
                 for (int c2 = 0; c2 < 8; ++c2)
-                    if (c2 < 4 || wide) rj[c2] = *reinterpret_cast<const double2 *>(Mj + 2 * (c2 ^ sj));
-                const double d = Mj[2 * ((j >> 1) ^ sj) + (j & 1)];
+                    if (c2 < 4 || wide) rj[c2] = *reinterpret_cast<const double2 *>(Mj + 2 * c2);
+                const double d = Mj[j];
                 const int ij = idx[j];
                 const bool ok = d > 1e-13 * G64s[ij * GS + ij];
                 if (on && !ok) rej = j;
                 const bool go = on && ok;
                 const double pv = rcp_d(go ? d : 1.0);
-                const int jc = 2 * ((j >> 1) ^ t) + (j & 1);    // column j inside my (swizzled) rows
-                double f0 = M0[jc] * pv, f1 = 0.0;
+                double f0 = M0[j] * pv, f1 = 0.0;
                 if (t == j) f0 = 1.0 - pv;                      // pivot row: m - (1 - p) m = p m
-                if (wide) { f1 = M1[jc] * pv; if (t + 8 == j) f1 = 1.0 - pv; }
+                if (wide) { f1 = M1[j] * pv; if (t + 8 == j) f1 = 1.0 - pv; }
                 __syncwarp();                                   // row j was read by everybody
                 if (go && t < k) {
 #pragma unroll
                     for (int c2 = 0; c2 < 8; ++c2) {
                         if (c2 < 4 || wide) {
-                            double2 m = *reinterpret_cast<double2 *>(M0 + 2 * (c2 ^ t));
+                            double2 m = *reinterpret_cast<double2 *>(M0 + 2 * c2);
                             m.x = fma(-f0, rj[c2].x, m.x); m.y = fma(-f0, rj[c2].y, m.y);
-                            *reinterpret_cast<double2 *>(M0 + 2 * (c2 ^ t)) = m;
+                            *reinterpret_cast<double2 *>(M0 + 2 * c2) = m;
                         }
                     }
-                    M0[jc] = (t == j) ? pv : -f0;
+                    M0[j] = (t == j) ? pv : -f0;
                 }
                 if (wide && go && t + 8 < k) {
 #pragma unroll
                     for (int c2 = 0; c2 < 8; ++c2) {
-                        double2 m = *reinterpret_cast<double2 *>(M1 + 2 * (c2 ^ t));
+                        double2 m = *reinterpret_cast<double2 *>(M1 + 2 * c2);
                         m.x = fma(-f1, rj[c2].x, m.x); m.y = fma(-f1, rj[c2].y, m.y);
-                        *reinterpret_cast<double2 *>(M1 + 2 * (c2 ^ t)) = m;
+                        *reinterpret_cast<double2 *>(M1 + 2 * c2) = m;
                     }
-                    M1[jc] = (t + 8 == j) ? pv : -f1;
+                    M1[j] = (t + 8 == j) ? pv : -f1;
                 }
                 __syncwarp();
             }
@@ -445,11 +444,11 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 for (int c2 = 0; c2 < 8; ++c2) {
                     if (c2 < 4 || wide) {
                         const double2 bb = *reinterpret_cast<const double2 *>(bR + 2 * c2);
-                        const double2 m = *reinterpret_cast<const double2 *>(M0 + 2 * (c2 ^ t));
+                        const double2 m = *reinterpret_cast<const double2 *>(M0 + 2 * c2);
                         q0 += m.x + m.y;
                         x0 = fma(m.x, bb.x, fma(m.y, bb.y, x0));
                         if (wide) {
-                            const double2 n = *reinterpret_cast<const double2 *>(M1 + 2 * (c2 ^ t));
+                            const double2 n = *reinterpret_cast<const double2 *>(M1 + 2 * c2);
                             q1 += n.x + n.y;
                             x1 = fma(n.x, bb.x, fma(n.y, bb.y, x1));
                         }
@@ -521,10 +520,10 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                     for (int c2 = 0; c2 < 8; ++c2) {
                         if (c2 < 4 || wide) {
                             const double2 qq = *reinterpret_cast<const double2 *>(qv + 2 * c2);
-                            const double2 m = *reinterpret_cast<const double2 *>(M0 + 2 * (c2 ^ t));
+                            const double2 m = *reinterpret_cast<const double2 *>(M0 + 2 * c2);
                             h0[2 * c2] = (float)fma(-u0, qq.x, m.x); h0[2 * c2 + 1] = (float)fma(-u0, qq.y, m.y);
                             if (wide) {
-                                const double2 n = *reinterpret_cast<const double2 *>(M1 + 2 * (c2 ^ t));
+                                const double2 n = *reinterpret_cast<const double2 *>(M1 + 2 * c2);
                                 h1[2 * c2] = (float)fma(-u1, qq.x, n.x); h1[2 * c2 + 1] = (float)fma(-u1, qq.y, n.y);
                             }
                         }
@@ -765,7 +764,7 @@ inline cudaError_t launch_finish_sweep_lq(const LibView &lv, const SolveParams &
                                           unsigned int *counter, unsigned int *overflow, cudaStream_t stream) {
     const size_t cta = (fs::cta_bytes(LQ) + 15) & ~(size_t)15;
     const size_t per_warp = 4 * (size_t)fs::PIX_BYTES;
-    int warps = (int)std::min<size_t>(16, (227 * 1024 - cta) / per_warp);
+    int warps = (int)std::min<size_t>(14, (227 * 1024 - cta) / per_warp);
     if (warps < 1) return cudaErrorInvalidConfiguration;
     const size_t smem = cta + per_warp * warps;
     cudaError_t e = cudaFuncSetAttribute(finish_sweep_kernel<LQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
