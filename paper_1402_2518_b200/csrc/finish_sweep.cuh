@@ -137,7 +137,7 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) {
 
 // LQ = float4 chunks of the spectrum per lane: L <= 32 LQ
 template <int LQ>
-__global__ void __maxnreg__(144)
+__global__ void __launch_bounds__(416, 1)
 finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter,
                     unsigned int *__restrict__ overflow /* [0] = count, [1 + i] = pixel */) {
     using namespace fs;
@@ -764,7 +764,7 @@ inline cudaError_t launch_finish_sweep_lq(const LibView &lv, const SolveParams &
                                           unsigned int *counter, unsigned int *overflow, cudaStream_t stream) {
     const size_t cta = (fs::cta_bytes(LQ) + 15) & ~(size_t)15;
     const size_t per_warp = 4 * (size_t)fs::PIX_BYTES;
-    int warps = (int)std::min<size_t>(14, (227 * 1024 - cta) / per_warp);
+    int warps = (int)std::min<size_t>(13, (227 * 1024 - cta) / per_warp);
     if (warps < 1) return cudaErrorInvalidConfiguration;
     const size_t smem = cta + per_warp * warps;
     cudaError_t e = cudaFuncSetAttribute(finish_sweep_kernel<LQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

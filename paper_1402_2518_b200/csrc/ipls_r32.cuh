@@ -42,9 +42,11 @@ namespace r32 {
 constexpr int R = 32;
 constexpr int GST = 36;        // padded row stride of G in shared memory (bank-conflict-free LDS.128)
 constexpr int XST = 56;        // one exchange line: 32 column entries + 8 x 2 right-hand sides + pad
-constexpr int LRS = 712;       // per-pixel factor-row area (704 used; 712 = 8 mod 32 spreads the pixels)
-constexpr int LR0 = 0, LR1 = 64, LR2 = 192, LR3 = 448;   // rows of slot s: 8 lanes x {1, 2, 4, 4} floats
-constexpr int PIXF = 2 * XST + LRS;   // floats per pixel
+constexpr int TBO = 2 * XST;   // diagonal blocks of -L: [4][8][8] floats (the centred spectrum during the projection)
+constexpr int RSO = TBO + 256; // reduce-scatter buffers: 2 x [8][12] floats
+constexpr int AGO = RSO + 192; // all-gather buffers: 2 x 8 floats
+constexpr int YCAP = 464;      // floats available to the centred spectrum (TBO .. end)
+constexpr int PIXF = 584;      // floats per pixel (576 used; 584 = 8 mod 32 spreads the pixels)
 constexpr int WARPS = 8;      // warps per CTA, one CTA per SM
 constexpr unsigned FULL = 0xffffffffu;
 
@@ -95,41 +97,74 @@ __host__ __device__ inline size_t smem_floats(int L) {
 // column j of the register-resident matrix (static j)
 #define LM_COL(s, j) (((j) & 1) ? m2[s][(j) >> 1].y : m2[s][(j) >> 1].x)
 
-// L z = r for ONE right-hand side, L unit lower, m2 holds -L (zeros on and above the diagonal of the
-// diagonal blocks): broadcast form, one shuffle per row.
-__device__ __forceinline__ void forward_subst1(const float2 (&m2)[4][16], float (&r)[4]) {
-#pragma unroll
-    for (int j = 0; j < 31; ++j) {
-        const int s0 = j >> 3, t0 = j & 7;
-        const float zj = __shfl_sync(FULL, r[s0], t0, 8);
-#pragma unroll
-        for (int s = s0; s < 4; ++s) r[s] = fmaf(LM_COL(s, j), zj, r[s]);
-    }
+// ---- exchanges inside a pixel group (8 lanes) through shared memory; consecutive calls alternate buffers
+// all-gather: every lane contributes one value and receives all eight
+__device__ __forceinline__ void allgather8(float *buf, int t, float v, float4 &lo, float4 &hi) {
+    buf[t] = v;
+    __syncwarp();
+    lo = *reinterpret_cast<const float4 *>(buf);
+    hi = *reinterpret_cast<const float4 *>(buf + 4);
+}
+// reduce-scatter: every lane contributes eight values, lane t receives the sum of the lanes' value t
+__device__ __forceinline__ float reduce_scatter8(float *buf, int t, const float2 (&c)[4]) {
+    *reinterpret_cast<float4 *>(buf + t * 12) = make_float4(c[0].x, c[0].y, c[1].x, c[1].y);
+    *reinterpret_cast<float4 *>(buf + t * 12 + 4) = make_float4(c[2].x, c[2].y, c[3].x, c[3].y);
+    __syncwarp();
+    const float s0 = buf[0 * 12 + t] + buf[1 * 12 + t], s1 = buf[2 * 12 + t] + buf[3 * 12 + t];
+    const float s2 = buf[4 * 12 + t] + buf[5 * 12 + t], s3 = buf[6 * 12 + t] + buf[7 * 12 + t];
+    return (s0 + s1) + (s2 + s3);
+}
+__device__ __forceinline__ float2 dot8(const float2 &p0, const float2 &p1, const float2 &p2, const float2 &p3,
+                                       const float4 &lo, const float4 &hi) {
+    float2 a = fma2(p0, make_float2(lo.x, lo.y), make_float2(0.0f, 0.0f));
+    float2 b = fma2(p2, make_float2(hi.x, hi.y), make_float2(0.0f, 0.0f));
+    a = fma2(p1, make_float2(lo.z, lo.w), a);
+    b = fma2(p3, make_float2(hi.z, hi.w), b);
+    return make_float2(a.x + b.x, a.y + b.y);
 }
 
-// L' x = y in place, broadcast form; row k of -L comes from the pixel's shared factor-row area
-__device__ __forceinline__ void backward_subst(const float *__restrict__ Lr, float (&y)[4], int t) {
+// Blocked substitutions.  L is unit lower, m2 holds -L (zeros on and above the diagonal of the 8 x 8
+// diagonal blocks T_s), ti[s] is row t of T_s^-1 (the lane's own row).  The dependent chain is 7
+// shared-memory exchanges instead of 31 shuffle steps.
+// L z = r:  z_s = T_s^-1 (r_s - sum_{s' < s} L_{s s'} z_{s'})
+__device__ __forceinline__ void forward_subst_blk(const float2 (&m2)[4][16], const float2 (&ti)[4][4],
+                                                  float (&r)[4], float *ag, int t) {
+    float4 zl[3], zh[3];
 #pragma unroll
-    for (int k = 31; k >= 1; --k) {
-        const int s0 = k >> 3, t0 = k & 7;
-        const float xk = __shfl_sync(FULL, y[s0], t0, 8);
-        const int pos = t ^ t0;
-        if (s0 == 3) {
-            const float4 v = *reinterpret_cast<const float4 *>(Lr + LR3 + t0 * 32 + 4 * pos);
-            y[0] = fmaf(v.x, xk, y[0]); y[1] = fmaf(v.y, xk, y[1]); y[2] = fmaf(v.z, xk, y[2]);
-            if (t0 > 0) y[3] = fmaf(v.w, xk, y[3]);
-        } else if (s0 == 2) {
-            const float4 v = *reinterpret_cast<const float4 *>(Lr + LR2 + t0 * 32 + 4 * pos);
-            y[0] = fmaf(v.x, xk, y[0]); y[1] = fmaf(v.y, xk, y[1]);
-            if (t0 > 0) y[2] = fmaf(v.z, xk, y[2]);
-        } else if (s0 == 1) {
-            const float2 v = *reinterpret_cast<const float2 *>(Lr + LR1 + t0 * 16 + 2 * pos);
-            y[0] = fmaf(v.x, xk, y[0]);
-            if (t0 > 0) y[1] = fmaf(v.y, xk, y[1]);
-        } else {
-            const float v = Lr[LR0 + t0 * 8 + pos];
-            y[0] = fmaf(v, xk, y[0]);
+    for (int s = 0; s < 4; ++s) {
+        float rp = r[s];
+#pragma unroll
+        for (int sp = 0; sp < s; ++sp) {
+            const float2 d = dot8(m2[s][4 * sp], m2[s][4 * sp + 1], m2[s][4 * sp + 2], m2[s][4 * sp + 3], zl[sp], zh[sp]);
+            rp += d.x + d.y;
         }
+        float4 gl, gh;
+        allgather8(ag, t, rp, gl, gh);
+        const float2 d = dot8(ti[s][0], ti[s][1], ti[s][2], ti[s][3], gl, gh);
+        r[s] = d.x + d.y;
+        if (s < 3) allgather8(ag + 8, t, r[s], zl[s], zh[s]);
+    }
+}
+// L' x = y:  x_s = T_s^-T (y_s - sum_{s' > s} L_{s' s}' x_{s'}); every lane adds its row's share, the
+// shares are summed by reduce-scatter
+__device__ __forceinline__ void backward_subst_blk(const float2 (&m2)[4][16], const float2 (&ti)[4][4],
+                                                   float (&y)[4], float *rs, int t) {
+    float2 acc[3][4];
+#pragma unroll
+    for (int s = 0; s < 3; ++s)
+#pragma unroll
+        for (int jp = 0; jp < 4; ++jp) acc[s][jp] = make_float2(0.0f, 0.0f);
+#pragma unroll
+    for (int s = 3; s >= 0; --s) {
+        if (s < 3) y[s] += reduce_scatter8(rs, t, acc[s]);
+        float2 c[4];
+#pragma unroll
+        for (int jp = 0; jp < 4; ++jp) c[jp] = make_float2(ti[s][jp].x * y[s], ti[s][jp].y * y[s]);
+        y[s] = reduce_scatter8(rs + 96, t, c);
+#pragma unroll
+        for (int sp = 0; sp < s; ++sp)
+#pragma unroll
+            for (int jp = 0; jp < 4; ++jp) acc[sp][jp] = fma2(y[s], m2[s][4 * sp + jp], acc[sp][jp]);
     }
 }
 
@@ -149,8 +184,10 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
     float *pix = cv + Lp + (size_t)((threadIdx.x >> 5) * 4 + g) * PIXF;
     float *xb0 = pix;                        // exchange line, buffer 0
     float *xb1 = pix + XST;                  // buffer 1
-    float *Lr = pix + 2 * XST;               // factor rows (backward substitution)
-    float *ybuf = Lr;                        // the centred spectrum lives here during the projection only
+    float *Tb = pix + TBO;                   // diagonal blocks of -L
+    float *rsb = pix + RSO;                  // reduce-scatter buffers
+    float *agb = pix + AGO;                  // all-gather buffers
+    float *ybuf = pix + TBO;                 // the centred spectrum lives here during the projection only
 
     // ---- once per CTA: stage the library data
     for (int e = threadIdx.x; e < R * R; e += blockDim.x) Gp[(e >> 5) * GST + (e & 31)] = lib.Gc[e];
@@ -385,19 +422,40 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                 m2[3][15].y = 0.0f;
             }
             if (__any_sync(0xffu << (8 * g), clamped)) flags |= LINMIN_INFO_CHOL_REGULARISED;
-            // ---- rows of -L to the shared factor-row area (chunk of reader lane t' at position t' ^ t)
+            // ---- diagonal blocks of -L to shared memory; every lane forms its row of T_s^-1:
+            //      x_j = [j == t] + sum_{i > j} x_i (-L)_{i j}  (row t of the inverse of a unit lower matrix)
 #pragma unroll
-            for (int tp = 0; tp < 8; ++tp) {
-                const int pos = tp ^ t;
-                Lr[LR0 + t * 8 + pos] = LM_COL(0, tp);
-                *reinterpret_cast<float2 *>(Lr + LR1 + t * 16 + 2 * pos) = make_float2(LM_COL(1, tp), LM_COL(1, 8 + tp));
-                *reinterpret_cast<float4 *>(Lr + LR2 + t * 32 + 4 * pos) =
-                    make_float4(LM_COL(2, tp), LM_COL(2, 8 + tp), LM_COL(2, 16 + tp), 0.0f);
-                *reinterpret_cast<float4 *>(Lr + LR3 + t * 32 + 4 * pos) =
-                    make_float4(LM_COL(3, tp), LM_COL(3, 8 + tp), LM_COL(3, 16 + tp), LM_COL(3, 24 + tp));
+            for (int s = 0; s < 4; ++s) {
+                *reinterpret_cast<float4 *>(Tb + s * 64 + t * 8) =
+                    make_float4(m2[s][4 * s].x, m2[s][4 * s].y, m2[s][4 * s + 1].x, m2[s][4 * s + 1].y);
+                *reinterpret_cast<float4 *>(Tb + s * 64 + t * 8 + 4) =
+                    make_float4(m2[s][4 * s + 2].x, m2[s][4 * s + 2].y, m2[s][4 * s + 3].x, m2[s][4 * s + 3].y);
             }
             __syncwarp();
-
+            float2 ti[4][4];
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                float T[8][8];
+#pragma unroll
+                for (int i = 1; i < 8; ++i) {
+                    const float4 u = *reinterpret_cast<const float4 *>(Tb + s * 64 + i * 8);
+                    T[i][0] = u.x; T[i][1] = u.y; T[i][2] = u.z; T[i][3] = u.w;
+                    if (i > 4) {
+                        const float4 v = *reinterpret_cast<const float4 *>(Tb + s * 64 + i * 8 + 4);
+                        T[i][4] = v.x; T[i][5] = v.y; T[i][6] = v.z; T[i][7] = v.w;
+                    }
+                }
+                float x[8];
+#pragma unroll
+                for (int j = 7; j >= 0; --j) {
+                    float v = (t == j) ? 1.0f : 0.0f;
+#pragma unroll
+                    for (int i = j + 1; i < 8; ++i) v = fmaf(x[i], T[i][j], v);
+                    x[j] = v;
+                }
+#pragma unroll
+                for (int jp = 0; jp < 4; ++jp) ti[s][jp] = make_float2(x[2 * jp], x[2 * jp + 1]);
+            }
             PH(3)
             // ---- predictor: M^-1 = L^-T D^-1 L^-1; nu eliminated through L^-1 1
             float sww = 0.0f, swz = 0.0f;
@@ -413,7 +471,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             float da[4], dl[4];
 #pragma unroll
             for (int s = 0; s < 4; ++s) da[s] = fmaf(-rr[s].x, dnu, rr[s].y) * dinv[s];
-            backward_subst(Lr, da, t);
+            backward_subst_blk(m2, ti, da, rsb, t);
             float mp = 0.0f, md = 0.0f;     // max of -da/a and -dl/lambda
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
@@ -438,7 +496,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                 cc[s] = fmaf(sg, mu, -da[s] * dl[s]);
                 r1[s] = fmaf(cc[s], ainv[s], -w[s]);
             }
-            forward_subst1(m2, r1);
+            forward_subst_blk(m2, ti, r1, agb, t);
             PH(5)
             swz = 0.0f;
 #pragma unroll
@@ -447,7 +505,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             dnu = (swz + rp) * rsww;
 #pragma unroll
             for (int s = 0; s < 4; ++s) da[s] = fmaf(-rr[s].x, dnu, r1[s]) * dinv[s];
-            backward_subst(Lr, da, t);
+            backward_subst_blk(m2, ti, da, rsb, t);
             mp = 0.0f; md = 0.0f;
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
@@ -486,7 +544,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
 #undef LM_COL
 
 inline bool ipls_r32_supported(int L) {
-    return r32::lpad(L) <= r32::LRS && r32::smem_floats(L) * sizeof(float) <= 226 * 1024;
+    return r32::lpad(L) <= r32::YCAP && r32::smem_floats(L) * sizeof(float) <= 226 * 1024;
 }
 
 // counter: device word, zero (the caller clears it on the stream before the launch)

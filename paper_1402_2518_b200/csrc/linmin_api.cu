@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -47,6 +48,7 @@ int cuda_status(cudaError_t e) {
         cudaError_t e__ = (call);                  \
         if (e__ != cudaSuccess) {                  \
             (void)cudaGetLastError();              \
+            if (getenv("LINMIN_DEBUG")) fprintf(stderr, "linmin: %s at %s:%d\n", cudaGetErrorString(e__), __FILE__, __LINE__); \
             return cuda_status(e__);               \
         }                                          \
     } while (0)
