@@ -17,6 +17,8 @@ struct LibView {
     const float *Gc;    // R x R fp32, Gc = Ac' Ac accumulated in fp64 (drives IPLS)
     const double *G64;  // R x R fp64, G = A' A (uncentred, exact data; drives the finish)
     float gdmax;        // max_i Gc[i][i]
+    const float *Gi;    // R x R fp32, (Gc + 1e-4 gdmax I)^-1 (start point of IPLS: regularised sum-constrained LS)
+    const float *Giq;   // R, row sums of Gi
 };
 
 struct SolveParams {

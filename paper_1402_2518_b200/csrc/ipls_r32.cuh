@@ -79,6 +79,12 @@ __device__ __forceinline__ float gsum(float v) {   // sum over the 8 lanes of a 
     v += __shfl_xor_sync(FULL, v, 4);
     return v;
 }
+__device__ __forceinline__ float gmin(float v) {
+    v = fminf(v, __shfl_xor_sync(FULL, v, 1));
+    v = fminf(v, __shfl_xor_sync(FULL, v, 2));
+    v = fminf(v, __shfl_xor_sync(FULL, v, 4));
+    return v;
+}
 __device__ __forceinline__ float gmax(float v) {
     v = fmaxf(v, __shfl_xor_sync(FULL, v, 1));
     v = fmaxf(v, __shfl_xor_sync(FULL, v, 2));
@@ -89,7 +95,7 @@ __device__ __forceinline__ float gmax(float v) {
 // shared-memory footprint in floats
 __host__ __device__ inline int lpad(int L) { return (L + 3) & ~3; }
 __host__ __device__ inline size_t smem_floats(int L) {
-    return (size_t)R * GST + R                 // Gp, row sums
+    return (size_t)2 * R * GST + 2 * R         // Gp, Gip, row sums of Gi (and their total)
            + (size_t)lpad(L) * R + lpad(L)      // Acp, c
            + (size_t)WARPS * 4 * PIXF;
 }
@@ -177,8 +183,9 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
     const int L = lib.L;
     const int Lp = lpad(L);
     float *Gp = smem;                        // [32][GST]
-    float *Grs = Gp + R * GST;               // [32] row sums of G
-    float *Acp = Grs + R;                    // [Lp][32]: Acp[l][t*4+s] = Ac[l][t+8s]
+    float *Gip = Gp + R * GST;               // [32][GST] inverse of the regularised G (start point)
+    float *Giq = Gip + R * GST;              // [32] row sums of Gi, [32] their total
+    float *Acp = Giq + 2 * R;                // [Lp][32]: Acp[l][t*4+s] = Ac[l][t+8s]
     float *cv = Acp + (size_t)Lp * R;        // [Lp]
     const int lane = threadIdx.x & 31, g = lane >> 3, t = lane & 7;
     float *pix = cv + Lp + (size_t)((threadIdx.x >> 5) * 4 + g) * PIXF;
@@ -190,17 +197,22 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
     float *ybuf = pix + TBO;                 // the centred spectrum lives here during the projection only
 
     // ---- once per CTA: stage the library data
-    for (int e = threadIdx.x; e < R * R; e += blockDim.x) Gp[(e >> 5) * GST + (e & 31)] = lib.Gc[e];
+    for (int e = threadIdx.x; e < R * R; e += blockDim.x) {
+        Gp[(e >> 5) * GST + (e & 31)] = lib.Gc[e];
+        Gip[(e >> 5) * GST + (e & 31)] = lib.Gi[e];
+    }
     for (int e = threadIdx.x; e < Lp * R; e += blockDim.x) {
         int l = e >> 5, c = e & 31, tt = c >> 2, s = c & 3;
         Acp[e] = (l < L) ? lib.Ac[(size_t)l * R + tt + 8 * s] : 0.0f;
     }
     for (int l = threadIdx.x; l < Lp; l += blockDim.x) cv[l] = (l < L) ? lib.c[l] : 0.0f;
     __syncthreads();
-    if (threadIdx.x < R) {
+    if (threadIdx.x < R) Giq[threadIdx.x] = lib.Giq[threadIdx.x];
+    __syncthreads();
+    if (threadIdx.x == 0) {
         float s = 0.0f;
-        for (int j = 0; j < R; ++j) s += Gp[threadIdx.x * GST + j];
-        Grs[threadIdx.x] = s;
+        for (int j = 0; j < R; ++j) s += Giq[j];
+        Giq[R] = s;
     }
     __syncthreads();
 
@@ -254,18 +266,84 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         float bmax = gmax(fmaxf(fmaxf(fabsf(b[0]), fabsf(b[1])), fmaxf(fabsf(b[2]), fabsf(b[3]))));
         const float sc = fmaxf(bmax, 1e-3f * gdmax);
 
-        // ---- start: a = 1/R, nu = 0, lambda = max(||G a - b||_inf, 1e-3 gdmax)
+        // ---- start (Mehrotra's heuristic on this QP): x = the sum-constrained LS point of the regularised
+        //      problem, lambda = its reduced gradient, both shifted into the interior
         float a[4], lam[4], w[4];
-        float g0 = 0.0f;
+        float nu, lam0;
+        {
+            __syncwarp();
 #pragma unroll
-        for (int s = 0; s < 4; ++s) {
-            a[s] = 1.0f / 32.0f;
-            g0 = fmaxf(g0, fabsf(Grs[t + 8 * s] * (1.0f / 32.0f) - b[s]));
+            for (int s = 0; s < 4; ++s) xb1[t + 8 * s] = b[s];
+            __syncwarp();
+            float2 x2[4];
+#pragma unroll
+            for (int s = 0; s < 4; ++s) x2[s] = make_float2(0.0f, 0.0f);
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const float4 b4 = *reinterpret_cast<const float4 *>(xb1 + 4 * c);
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    const float4 g4 = *reinterpret_cast<const float4 *>(Gip + (t + 8 * s) * GST + 4 * c);
+                    x2[s] = fma2(make_float2(g4.x, g4.y), make_float2(b4.x, b4.y), x2[s]);
+                    x2[s] = fma2(make_float2(g4.z, g4.w), make_float2(b4.z, b4.w), x2[s]);
+                }
+            }
+            float x[4], q[4], sx = 0.0f;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) { x[s] = x2[s].x + x2[s].y; q[s] = Giq[t + 8 * s]; sx += x[s]; }
+            sx = gsum(sx);
+            const float mu0 = (sx - 1.0f) / Giq[R];
+#pragma unroll
+            for (int s = 0; s < 4; ++s) { x[s] = fmaf(-mu0, q[s], x[s]); xb0[t + 8 * s] = x[s]; }
+            __syncwarp();
+#pragma unroll
+            for (int s = 0; s < 4; ++s) x2[s] = make_float2(0.0f, 0.0f);
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const float4 b4 = *reinterpret_cast<const float4 *>(xb0 + 4 * c);
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    const float4 g4 = *reinterpret_cast<const float4 *>(Gp + (t + 8 * s) * GST + 4 * c);
+                    x2[s] = fma2(make_float2(g4.x, g4.y), make_float2(b4.x, b4.y), x2[s]);
+                    x2[s] = fma2(make_float2(g4.z, g4.w), make_float2(b4.z, b4.w), x2[s]);
+                }
+            }
+            float gx = 0.0f, mnx = INFINITY, mng = INFINITY;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                lam[s] = x2[s].x + x2[s].y - b[s];          // gradient at x
+                gx = fmaf(lam[s], x[s], gx);
+                mnx = fminf(mnx, x[s]); mng = fminf(mng, lam[s]);
+            }
+            gx = gsum(gx); mnx = gmin(mnx); mng = gmin(mng);
+            nu = -gx;
+            const float dp = fmaxf(-mnx, 0.0f), dd = fmaxf(-(mng + nu), 0.0f);
+            float xl = 0.0f, sl = 0.0f, sxx = 0.0f;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                x[s] += dp; lam[s] += nu + dd;
+                xl = fmaf(x[s], lam[s], xl); sl += lam[s]; sxx += x[s];
+            }
+            xl = gsum(xl); sl = gsum(sl); sxx = gsum(sxx);
+            const float dp2 = 0.05f * xl / fmaxf(sl, 1e-30f), dd2 = 0.05f * xl / fmaxf(sxx, 1e-30f);
+            float sa = 0.0f, lm = 0.0f;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                a[s] = x[s] + dp2 + 1e-3f;
+                lam[s] = lam[s] + dd2 + 1e-4f * sc;
+                sa += a[s]; lm = fmaxf(lm, lam[s]);
+            }
+            sa = gsum(sa); lam0 = gmax(lm);
+            const float rsa = 1.0f / sa;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) a[s] *= rsa;
+            if (!(lam0 > 0.0f) || !isfinite(lam0) || !isfinite(sa)) {     // degenerate data: fall back to the flat start
+                lam0 = fmaxf(bmax, 1e-3f * gdmax);
+#pragma unroll
+                for (int s = 0; s < 4; ++s) { a[s] = 1.0f / 32.0f; lam[s] = lam0; }
+                nu = 0.0f;
+            }
         }
-        const float lam0 = fmaxf(gmax(g0), 1e-3f * gdmax);
-#pragma unroll
-        for (int s = 0; s < 4; ++s) lam[s] = lam0;
-        float nu = 0.0f;
         int iters = 0, flags = bad ? LINMIN_INFO_NONFINITE_INPUT : 0;
         bool done = false;
 

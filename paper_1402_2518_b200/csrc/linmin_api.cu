@@ -26,7 +26,7 @@ struct linmin_library {
     int device = 0;
     int sm_count = 0;
     cudaStream_t stream = nullptr;   // stream the handle was created on (frees are ordered on it)
-    float *A = nullptr, *Ac = nullptr, *c = nullptr, *Gc = nullptr;
+    float *A = nullptr, *Ac = nullptr, *c = nullptr, *Gc = nullptr, *Gi = nullptr, *Giq = nullptr;
     double *G64 = nullptr;
     float gdmax = 0.0f;
     mutable int last_launches = 0;
@@ -100,7 +100,7 @@ int check_sizes(int64_t N, int L, int R) {
 LibView view_of(const linmin_library *lib) {
     LibView v;
     v.L = lib->L; v.R = lib->R; v.A = lib->A; v.Ac = lib->Ac; v.c = lib->c; v.Gc = lib->Gc;
-    v.G64 = lib->G64; v.gdmax = lib->gdmax;
+    v.G64 = lib->G64; v.gdmax = lib->gdmax; v.Gi = lib->Gi; v.Giq = lib->Giq;
     return v;
 }
 
@@ -237,6 +237,48 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
     for (int i = 0; i < R; ++i) gd = std::max(gd, hG[(size_t)i * R + i]);
     if (!(gd > 0.0f)) gd = 1.0f;   // all endmembers identical: any point of the simplex is optimal
     lib->gdmax = gd;
+    {   // start point data of IPLS: inverse of the regularised centred Gram matrix (fp64 Gauss-Jordan with
+        // partial pivoting on the host, once per library) and its row sums
+        const double delta = 1e-4 * (double)gd;
+        std::vector<double> M((size_t)R * 2 * R, 0.0);
+        for (int i = 0; i < R; ++i) {
+            for (int j = 0; j < R; ++j) M[(size_t)i * 2 * R + j] = (double)hG[(size_t)i * R + j];
+            M[(size_t)i * 2 * R + i] += delta;
+            M[(size_t)i * 2 * R + R + i] = 1.0;
+        }
+        for (int j = 0; j < R; ++j) {
+            int piv = j;
+            for (int i = j + 1; i < R; ++i)
+                if (std::fabs(M[(size_t)i * 2 * R + j]) > std::fabs(M[(size_t)piv * 2 * R + j])) piv = i;
+            if (piv != j)
+                for (int c2 = 0; c2 < 2 * R; ++c2) std::swap(M[(size_t)j * 2 * R + c2], M[(size_t)piv * 2 * R + c2]);
+            double d = M[(size_t)j * 2 * R + j];
+            if (!(std::fabs(d) > 0.0)) d = delta;
+            const double pinv = 1.0 / d;
+            for (int c2 = 0; c2 < 2 * R; ++c2) M[(size_t)j * 2 * R + c2] *= pinv;
+            for (int i = 0; i < R; ++i) {
+                if (i == j) continue;
+                const double f = M[(size_t)i * 2 * R + j];
+                if (f == 0.0) continue;
+                for (int c2 = 0; c2 < 2 * R; ++c2) M[(size_t)i * 2 * R + c2] -= f * M[(size_t)j * 2 * R + c2];
+            }
+        }
+        std::vector<float> hGi(RR), hq(R);
+        for (int i = 0; i < R; ++i) {
+            double q = 0.0;
+            for (int j = 0; j < R; ++j) {
+                const double v = 0.5 * (M[(size_t)i * 2 * R + R + j] + M[(size_t)j * 2 * R + R + i]);
+                hGi[(size_t)i * R + j] = (float)v;
+                q += v;
+            }
+            hq[i] = (float)q;
+        }
+        CKF(cudaMallocAsync((void **)&lib->Gi, RR * sizeof(float), stream));
+        CKF(cudaMallocAsync((void **)&lib->Giq, (size_t)R * sizeof(float), stream));
+        CKF(cudaMemcpyAsync(lib->Gi, hGi.data(), RR * sizeof(float), cudaMemcpyHostToDevice, stream));
+        CKF(cudaMemcpyAsync(lib->Giq, hq.data(), (size_t)R * sizeof(float), cudaMemcpyHostToDevice, stream));
+        CKF(cudaStreamSynchronize(stream));
+    }
     if (R > L) rc = LINMIN_WARN_RANK_DEFICIENT;
     *out = lib;
     return rc;
@@ -292,6 +334,8 @@ void linmin_library_destroy(linmin_library *lib) {
     if (lib->Ac) cudaFreeAsync(lib->Ac, s);
     if (lib->c) cudaFreeAsync(lib->c, s);
     if (lib->Gc) cudaFreeAsync(lib->Gc, s);
+    if (lib->Gi) cudaFreeAsync(lib->Gi, s);
+    if (lib->Giq) cudaFreeAsync(lib->Giq, s);
     if (lib->G64) cudaFreeAsync(lib->G64, s);
     for (int i = 0; i < 3; ++i) if (lib->ev[i]) cudaEventDestroy(lib->ev[i]);
     (void)cudaGetLastError();
