@@ -42,11 +42,11 @@ namespace r32 {
 constexpr int R = 32;
 constexpr int GST = 36;        // padded row stride of G in shared memory (bank-conflict-free LDS.128)
 constexpr int XST = 56;        // one exchange line: 32 column entries + 8 x 2 right-hand sides + pad
-constexpr int TBO = 2 * XST;   // diagonal blocks of -L: [4][8][8] floats (the centred spectrum during the projection)
+constexpr int TBO = 2 * XST;   // diagonal blocks of -L: [4][8][8] floats
 constexpr int RSO = TBO + 256; // reduce-scatter buffers: 2 x [8][12] floats
 constexpr int AGO = RSO + 192; // all-gather buffers: 2 x 8 floats
-constexpr int YCAP = 464;      // floats available to the centred spectrum (TBO .. end)
-constexpr int PIXF = 584;      // floats per pixel (576 used; 584 = 8 mod 32 spreads the pixels)
+constexpr int PIXF = 584;      // fixed floats per pixel (576 used; 584 = 8 mod 32 spreads the pixels),
+                               // followed by two spectrum buffers of lpad(L) floats (this pixel, the next one)
 constexpr int WARPS = 8;      // warps per CTA, one CTA per SM
 constexpr unsigned FULL = 0xffffffffu;
 
@@ -97,7 +97,7 @@ __host__ __device__ inline int lpad(int L) { return (L + 3) & ~3; }
 __host__ __device__ inline size_t smem_floats(int L) {
     return (size_t)2 * R * GST + 2 * R         // Gp, Gip, row sums of Gi (and their total)
            + (size_t)lpad(L) * R + lpad(L)      // Acp, c
-           + (size_t)WARPS * 4 * PIXF;
+           + (size_t)WARPS * 4 * (PIXF + 2 * lpad(L));
 }
 
 // column j of the register-resident matrix (static j)
@@ -188,13 +188,14 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
     float *Acp = Giq + 2 * R;                // [Lp][32]: Acp[l][t*4+s] = Ac[l][t+8s]
     float *cv = Acp + (size_t)Lp * R;        // [Lp]
     const int lane = threadIdx.x & 31, g = lane >> 3, t = lane & 7;
-    float *pix = cv + Lp + (size_t)((threadIdx.x >> 5) * 4 + g) * PIXF;
+    float *pix = cv + Lp + (size_t)((threadIdx.x >> 5) * 4 + g) * (PIXF + 2 * Lp);
     float *xb0 = pix;                        // exchange line, buffer 0
     float *xb1 = pix + XST;                  // buffer 1
     float *Tb = pix + TBO;                   // diagonal blocks of -L
     float *rsb = pix + RSO;                  // reduce-scatter buffers
     float *agb = pix + AGO;                  // all-gather buffers
-    float *ybuf = pix + TBO;                 // the centred spectrum lives here during the projection only
+    float *yb0 = pix + PIXF;                 // spectrum buffers: the current pixel and the prefetched next one
+    float *yb1 = yb0 + Lp;
 
     // ---- once per CTA: stage the library data
     for (int e = threadIdx.x; e < R * R; e += blockDim.x) {
@@ -224,25 +225,51 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
 #pragma unroll
     for (int jp = 0; jp < 4; ++jp) e2[jp] = make_float2((t == 2 * jp) ? 1.0f : 0.0f, (t == 2 * jp + 1) ? 1.0f : 0.0f);
 
+    // spectra arrive by cp.async (16 B per lane and step) one task ahead of their use
+    const bool vec_ok = ((L & 3) == 0) && ((prm.ldY & 3) == 0) && ((reinterpret_cast<uintptr_t>(prm.Y) & 15) == 0);
+    // work counter: the atomic for task i + 2 is issued at the start of task i and read at its end
+    auto take_ticket = [&]() -> unsigned int { return (lane == 0) ? atomicAdd(counter, 1u) : 0u; };
+    auto prefetch = [&](unsigned int grp_, float *dst) {
+        const int64_t q0 = (int64_t)grp_ * 4;
+        if (q0 >= prm.N) return;
+        const int64_t q = (q0 + g < prm.N) ? (q0 + g) : (prm.N - 1);
+        const float *src = prm.Y + q * prm.ldY;
+        if (vec_ok) {
+            for (int l = 4 * t; l < Lp; l += 32) {
+                const unsigned sa = (unsigned)__cvta_generic_to_shared(dst + l);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(src + l) : "memory");
+            }
+        } else {
+            for (int l = t; l < Lp; l += 8) dst[l] = (l < L) ? src[l] : 0.0f;
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
     PH_DECL
+    unsigned int grp = __shfl_sync(FULL, take_ticket(), 0);
+    unsigned int grp_next = __shfl_sync(FULL, take_ticket(), 0);
+    prefetch(grp, yb0);
+    int par = 0;
     while (true) {
         PH(8)
-        unsigned int grp = 0;
-        if (lane == 0) grp = atomicAdd(counter, 1u);
-        grp = __shfl_sync(FULL, grp, 0);
         const int64_t p0 = (int64_t)grp * 4;
         if (p0 >= prm.N) break;
         const bool valid = (p0 + g) < prm.N;
         const int64_t p = valid ? (p0 + g) : (prm.N - 1);
-
-        // ---- load the spectrum (8 lanes x 4 B = one 32 B sector per step), centre, flag non-finite
-        const float *y = prm.Y + p * prm.ldY;
-        bool bad = false;
+        float *ybuf = par ? yb1 : yb0;
+        const unsigned int ticket = take_ticket();
+        prefetch(grp_next, par ? yb0 : yb1);
+        if ((int64_t)grp_next * 4 < prm.N) asm volatile("cp.async.wait_group 1;" ::: "memory");
+        else asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncwarp();
-        for (int l = t; l < Lp; l += 8) {
-            float yv = (l < L) ? y[l] : 0.0f;
-            bad |= !isfinite(yv);
-            ybuf[l] = yv - cv[l];
+
+        // ---- centre my chunks of the spectrum in place, flag non-finite values
+        bool bad = false;
+        for (int l = 4 * t; l < Lp; l += 32) {
+            float4 y4 = *reinterpret_cast<const float4 *>(ybuf + l);
+            const float4 c4 = *reinterpret_cast<const float4 *>(cv + l);
+            bad |= !isfinite(y4.x) || !isfinite(y4.y) || !isfinite(y4.z) || !isfinite(y4.w);
+            y4.x -= c4.x; y4.y -= c4.y; y4.z -= c4.z; y4.w -= c4.w;
+            *reinterpret_cast<float4 *>(ybuf + l) = y4;
         }
         bad = __any_sync(0xffu << (8 * g), bad);
         __syncwarp();
@@ -251,16 +278,21 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
 
         // ---- projection b = Ac'(y - c)
         float2 b01 = make_float2(0.0f, 0.0f), b23 = make_float2(0.0f, 0.0f);
-        for (int l4 = 0; l4 < Lp; l4 += 4) {
-            const float4 y4 = *reinterpret_cast<const float4 *>(ybuf + l4);
-            const float4 a0 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 0) * R + t * 4);
-            const float4 a1 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 1) * R + t * 4);
-            const float4 a2 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 2) * R + t * 4);
-            const float4 a3 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 3) * R + t * 4);
-            b01 = fma2(y4.x, make_float2(a0.x, a0.y), b01); b23 = fma2(y4.x, make_float2(a0.z, a0.w), b23);
-            b01 = fma2(y4.y, make_float2(a1.x, a1.y), b01); b23 = fma2(y4.y, make_float2(a1.z, a1.w), b23);
-            b01 = fma2(y4.z, make_float2(a2.x, a2.y), b01); b23 = fma2(y4.z, make_float2(a2.z, a2.w), b23);
-            b01 = fma2(y4.w, make_float2(a3.x, a3.y), b01); b23 = fma2(y4.w, make_float2(a3.z, a3.w), b23);
+        {
+            float2 c01 = make_float2(0.0f, 0.0f), c23 = make_float2(0.0f, 0.0f);
+#pragma unroll 4
+            for (int l4 = 0; l4 < Lp; l4 += 4) {
+                const float4 y4 = *reinterpret_cast<const float4 *>(ybuf + l4);
+                const float4 a0 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 0) * R + t * 4);
+                const float4 a1 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 1) * R + t * 4);
+                const float4 a2 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 2) * R + t * 4);
+                const float4 a3 = *reinterpret_cast<const float4 *>(Acp + (size_t)(l4 + 3) * R + t * 4);
+                b01 = fma2(y4.x, make_float2(a0.x, a0.y), b01); b23 = fma2(y4.x, make_float2(a0.z, a0.w), b23);
+                c01 = fma2(y4.y, make_float2(a1.x, a1.y), c01); c23 = fma2(y4.y, make_float2(a1.z, a1.w), c23);
+                b01 = fma2(y4.z, make_float2(a2.x, a2.y), b01); b23 = fma2(y4.z, make_float2(a2.z, a2.w), b23);
+                c01 = fma2(y4.w, make_float2(a3.x, a3.y), c01); c23 = fma2(y4.w, make_float2(a3.z, a3.w), c23);
+            }
+            b01.x += c01.x; b01.y += c01.y; b23.x += c23.x; b23.y += c23.y;
         }
         const float b[4] = {b01.x, b01.y, b23.x, b23.y};
         float bmax = gmax(fmaxf(fmaxf(fabsf(b[0]), fabsf(b[1])), fmaxf(fabsf(b[2]), fabsf(b[3]))));
@@ -292,7 +324,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
 #pragma unroll
             for (int s = 0; s < 4; ++s) { x[s] = x2[s].x + x2[s].y; q[s] = Giq[t + 8 * s]; sx += x[s]; }
             sx = gsum(sx);
-            const float mu0 = (sx - 1.0f) / Giq[R];
+            const float mu0 = (sx - 1.0f) * rcp_approx(Giq[R]);
 #pragma unroll
             for (int s = 0; s < 4; ++s) { x[s] = fmaf(-mu0, q[s], x[s]); xb0[t + 8 * s] = x[s]; }
             __syncwarp();
@@ -325,7 +357,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                 xl = fmaf(x[s], lam[s], xl); sl += lam[s]; sxx += x[s];
             }
             xl = gsum(xl); sl = gsum(sl); sxx = gsum(sxx);
-            const float dp2 = 0.05f * xl / fmaxf(sl, 1e-30f), dd2 = 0.05f * xl / fmaxf(sxx, 1e-30f);
+            const float dp2 = 0.05f * xl * rcp_approx(fmaxf(sl, 1e-30f)), dd2 = 0.05f * xl * rcp_approx(fmaxf(sxx, 1e-30f));
             float sa = 0.0f, lm = 0.0f;
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
@@ -615,6 +647,9 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             if (prm.info && t == 0) prm.info[p] = flags | (iters << 8);
         }
         __syncwarp();
+        grp = grp_next;
+        grp_next = __shfl_sync(FULL, ticket, 0);
+        par ^= 1;
     }
     PH(8)
     PH_FLUSH
@@ -622,7 +657,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
 #undef LM_COL
 
 inline bool ipls_r32_supported(int L) {
-    return r32::lpad(L) <= r32::YCAP && r32::smem_floats(L) * sizeof(float) <= 226 * 1024;
+    return r32::smem_floats(L) * sizeof(float) <= 226 * 1024;
 }
 
 // counter: device word, zero (the caller clears it on the stream before the launch)
