@@ -186,14 +186,48 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
     double *M0 = Md + t * MS;          // my rows of the swept matrix
     double *M1 = Md + (t + 8) * MS;
 
+    // Work unit of a warp: a chunk of 32 consecutive pixels.  Lane i counts the support of pixel i from
+    // the IPLS iterate, the 32 counts are ranked (ties by lane), and the chunk is processed as 8 tasks
+    // of 4 pixels with neighbouring support sizes: the k-bounded loops of a task then run (almost)
+    // without padding (mean of the warp maximum 11.1 -> 8 on config 4).
+    int *perm = (int *)((unsigned char *)(At32 + (size_t)RP * RS) + (size_t)(blockDim.x >> 5) * 4 * PIX_BYTES) + warp * 32;
     while (true) {
-        unsigned int grp = 0;
-        if (lane == 0) grp = atomicAdd(counter, 1u);
-        grp = __shfl_sync(FULL, grp, 0);
-        const int64_t p0 = (int64_t)grp * 4;
-        if (p0 >= prm.N) break;
-        const bool valid = (p0 + g) < prm.N;
-        const int64_t p = valid ? (p0 + g) : (prm.N - 1);
+        unsigned int chunk = 0;
+        if (lane == 0) chunk = atomicAdd(counter, 1u);
+        chunk = __shfl_sync(FULL, chunk, 0);
+        const int64_t pbase = (int64_t)chunk * 32;
+        if (pbase >= prm.N) break;
+        {
+            int kc = -1;
+            if (pbase + lane < prm.N) {
+                const float *cp = prm.coeffs + (pbase + lane) * R;
+                kc = 0;
+                if (cvec_ok) {
+                    for (int i = 0; i < R; i += 4) {
+                        const float4 c4 = *reinterpret_cast<const float4 *>(cp + i);
+                        kc += (c4.x > LINMIN_SUPPORT_THRESHOLD) + (c4.y > LINMIN_SUPPORT_THRESHOLD) +
+                              (c4.z > LINMIN_SUPPORT_THRESHOLD) + (c4.w > LINMIN_SUPPORT_THRESHOLD);
+                    }
+                } else {
+                    for (int i = 0; i < R; ++i) kc += cp[i] > LINMIN_SUPPORT_THRESHOLD;
+                }
+            }
+            int pos = 0;
+#pragma unroll
+            for (int d = 1; d < 32; ++d) {
+                const int j = (lane + d) & 31;
+                const int kj = __shfl_sync(FULL, kc, j);
+                pos += (kj > kc) || (kj == kc && j < lane);
+            }
+            __syncwarp();
+            perm[pos] = lane;
+            __syncwarp();
+        }
+      for (int task = 0; task < 8; ++task) {
+        const int64_t p_raw = pbase + perm[4 * task + g];
+        if (pbase + perm[4 * task] >= prm.N) break;          // sorted: invalid pixels (k = -1) come last
+        const bool valid = p_raw < prm.N;
+        const int64_t p = valid ? p_raw : (prm.N - 1);
         float *cout = prm.coeffs + p * R;
         int info = prm.info ? prm.info[p] : 0;
 
@@ -754,6 +788,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             prm.info[p] = (info & 0xffff) | (pv << 16) | (k << 24);
         }
         __syncwarp();
+      }
     }
 }
 
@@ -763,14 +798,14 @@ template <int LQ>
 inline cudaError_t launch_finish_sweep_lq(const LibView &lv, const SolveParams &prm, int sm_count,
                                           unsigned int *counter, unsigned int *overflow, cudaStream_t stream) {
     const size_t cta = (fs::cta_bytes(LQ) + 15) & ~(size_t)15;
-    const size_t per_warp = 4 * (size_t)fs::PIX_BYTES;
+    const size_t per_warp = 4 * (size_t)fs::PIX_BYTES + 128;     // scratch of 4 pixels + the chunk permutation
     int warps = (int)std::min<size_t>(13, (227 * 1024 - cta) / per_warp);
     if (warps < 1) return cudaErrorInvalidConfiguration;
     const size_t smem = cta + per_warp * warps;
     cudaError_t e = cudaFuncSetAttribute(finish_sweep_kernel<LQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    const int64_t groups = (prm.N + 3) / 4;
-    const int64_t need = (groups + warps - 1) / warps;
+    const int64_t chunks = (prm.N + 31) / 32;
+    const int64_t need = (chunks + warps - 1) / warps;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, sm_count));
     finish_sweep_kernel<LQ><<<grid, warps * 32, smem, stream>>>(lv, prm, counter, overflow);
     return cudaGetLastError();
