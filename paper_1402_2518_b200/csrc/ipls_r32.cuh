@@ -1,24 +1,30 @@
-// ipls_r32.cuh -- register-blocked projection + IPLS kernel for R = 32 endmembers (sm_100a), v3.
+// ipls_r32.cuh -- register-blocked projection + IPLS kernel for R = 32 endmembers (sm_100a), v4.
 //
 // Same iteration as ipls_generic.cuh (Mehrotra predictor-corrector on the centred normal equations;
 // PAPER.md:71-73 names IPLS and prints no steps -- DESIGN.md reading R1), mapped to the hardware:
 //
-//   * 8 lanes cooperate on one pixel, 4 pixels per warp.  Lane t of a group owns rows
-//     i = t + 8 s (s = 0..3, cyclic) of the 32 x 32 Newton matrix M = G + diag(lambda/a): row i is
-//     kept in REGISTERS up to column 8 s + 7, as 40 packed pairs (80 registers), so that the
-//     rank-one updates are FFMA2 (fma.rn.f32x2: two FMAs per issue slot).
+//   * 8 lanes cooperate on one pixel, 4 pixels per warp, 8 warps per SM (255 registers, no spill traffic
+//     on the dependent chains).  Lane t of a group owns rows i = t + 8 s (s = 0..3, cyclic) of the
+//     32 x 32 Newton matrix M = G + diag(lambda/a): row i is kept in REGISTERS up to column 8 s + 7, as
+//     40 packed pairs (80 registers), so that the rank-one updates are FFMA2 (fma.rn.f32x2).
+//   * Start point (Mehrotra's heuristic for this QP): the sum-constrained LS point of the regularised
+//     problem, x = Gi b - q (1'Gi b - 1)/(1'q) with Gi = (G + 1e-4 max G_ii I)^-1 precomputed per library,
+//     and its reduced gradient as multipliers, both shifted into the interior.  5.8 iterations on the
+//     OMEGA-like cubes instead of 10.1 from the barycentre.
 //   * Square-root-free Cholesky M = L D L', right-looking, fully unrolled (static register indices).
 //     Step k: every lane puts its raw entries of column k on a double-buffered, bank-padded shared
 //     line, one __syncwarp, every lane reads the column back with LDS.128 (16 FMAs per load) and forms
-//     1/d_k itself: no shuffle, no square root on the dependent chain of a step.
+//     1/d_k itself.  Column k + 1 is updated and exchanged BEFORE the rest of the rank-one update of
+//     step k (look-ahead), so the shared-memory round trip overlaps the FFMA2 stream.
 //   * The forward substitution of the predictor (right-hand sides 1 and -w) is fused into the
 //     factorisation: the two right-hand sides ride along as a packed pair per row.
-//   * Backward substitutions in broadcast form: after the factorisation each lane writes its rows of
-//     L (xor-swizzled, conflict-free) to a per-pixel shared area; step k is one shuffle (x_k), one
-//     LDS (row k of L at my columns) and <= 4 FMAs -- instead of a 3-shuffle reduction per row.
-//   * G (padded rows), the centred library (re-laid out so that a lane's four rows are one LDS.128)
-//     and the channel means live in shared memory, loaded once per CTA (one CTA of 12 warps per SM);
-//     warps run independently and fetch groups of 4 pixels from a global atomic counter.
+//   * Blocked substitutions: every lane forms its row of the inverse of the four 8 x 8 diagonal blocks
+//     of L; a substitution is then 7 exchanges through shared memory (all-gather in the forward,
+//     reduce-scatter in the backward direction) instead of a 31-step shuffle chain.
+//   * G, Gi (padded rows), the centred library (re-laid out so that a lane's four rows are one LDS.128)
+//     and the channel means live in shared memory, loaded once per CTA; warps run independently on
+//     groups of 4 pixels taken from a global atomic counter; the spectrum of the NEXT group is fetched
+//     with cp.async while the current one iterates.
 //
 // Algorithmic work per pixel: 2 L R + it (R^3/3 + 8 R^2 + 30 R) flops.
 #pragma once
