@@ -11,7 +11,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblinmin.so")
-SOURCES = ["linmin_api.cu"]
+# source -> extra flags of its translation unit
+SOURCES = {"linmin_api.cu": [], "finish_sweep.cu": []}
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false"]
 
@@ -31,8 +32,21 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     if verbose:
         flags += ["-Xptxas", "-v"]
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc] + flags + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES] + ["-lcudart"]
-    subprocess.check_call(cmd)
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    cflags = [f for f in flags if f != "-shared"]
+    objs = []
+    procs = []
+    for src, extra in SOURCES.items():
+        obj = os.path.join(objdir, src.replace(".cu", f".{os.getpid()}.o"))
+        objs.append(obj)
+        procs.append(subprocess.Popen([nvcc] + cflags + extra + ["-c", "-o", obj, os.path.join(CSRC, src)]))
+    for pr in procs:
+        if pr.wait() != 0:
+            raise subprocess.CalledProcessError(pr.returncode, pr.args)
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp] + objs + ["-lcudart"])
+    for o in objs:
+        os.remove(o)
     os.replace(tmp, LIB)
     return LIB
 

@@ -6,6 +6,9 @@
 
 #include "../../include/linmin.h"
 
+// an endmember belongs to the initial support of the finish when its IPLS coefficient exceeds this
+#define LINMIN_SUPPORT_THRESHOLD 1e-4f
+
 namespace linmin {
 
 // Device-side view of the once-per-library precompute.

@@ -22,7 +22,6 @@
 
 namespace linmin {
 
-#define LINMIN_SUPPORT_THRESHOLD 1e-4f
 
 __host__ __device__ inline size_t finish_warp_bytes(int L, int R, int KMAX) {
     size_t dbl = (size_t)KMAX * (KMAX + 1) / 2   // Lf

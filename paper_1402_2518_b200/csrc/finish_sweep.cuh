@@ -1,5 +1,5 @@
 // finish_sweep.cuh -- exact finish + uncertainty + residual for R <= 32, L <= 256 (sm_100a), v3 of the
-// throughput path of SURVEY.md 8(a) a3-a6 (replaces finish8.cuh on that path).
+// throughput path of SURVEY.md 8(a) a3-a6 (replaces the round-1 finish8 kernel on that path).
 //
 // Same mathematics and the same active-set logic as finish.cuh (read its header: PAPER.md:54-68
 // optimality conditions, PAPER.md:88 uncertainty reading R3, PAPER.md:143 RMS reading R8).  What changed
@@ -16,7 +16,6 @@
 // support members (ranks) t and t + 8, and endmembers 4 t + q.
 #pragma once
 #include "common.cuh"
-#include "finish.cuh"
 
 namespace linmin {
 namespace fs {
@@ -137,7 +136,7 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) {
 
 // LQ = float4 chunks of the spectrum per lane: L <= 32 LQ
 template <int LQ>
-__global__ void __launch_bounds__(416, 1)
+__global__ void __launch_bounds__(384, 1)
 finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter,
                     unsigned int *__restrict__ overflow /* [0] = count, [1 + i] = pixel */) {
     using namespace fs;
@@ -249,6 +248,27 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             for (int q = 0; q < 4; ++q) bad |= !isfinite(yv[4 * v + q]);
         }
         bad = ((__ballot_sync(FULL, bad) >> (8 * g)) & 0xffu) != 0u;
+        // ---- noise std -> registers now, so that the load is long done when the uncertainty pass needs it
+        float2 sv[NC / 2];
+        bool sbad = false;
+        if (prm.coeff_sigma && prm.has_sigma) {
+            const float *sp = prm.sigma + p * prm.sigma_stride;
+#pragma unroll
+            for (int v = 0; v < LQ; ++v) {
+                const int l = 4 * (t + 8 * v);
+                float4 t4;
+                if (svec_ok && l + 3 < L) {
+                    t4 = *reinterpret_cast<const float4 *>(sp + l);
+                } else {
+                    t4.x = (l + 0 < L) ? sp[l + 0] : 1.0f; t4.y = (l + 1 < L) ? sp[l + 1] : 1.0f;
+                    t4.z = (l + 2 < L) ? sp[l + 2] : 1.0f; t4.w = (l + 3 < L) ? sp[l + 3] : 1.0f;
+                }
+                sv[2 * v] = make_float2(t4.x, t4.y); sv[2 * v + 1] = make_float2(t4.z, t4.w);
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < NC / 2; ++c) sv[c] = make_float2(1.0f, 1.0f);
+        }
 
         // ---- initial support from the IPLS iterate; lane t looks at endmembers 4 t + q
         // st: 0 solving, 1 optimal, 2 fallback (feasible point, not certified), 3 nothing to write here
@@ -605,7 +625,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 }
                 // ---- g_i = A_i'r for every endmember (FFMA2 over my channels), partial sums exchanged
                 //      through Ex[lane][chunk ^ lane]; lane t ends with endmembers 4 t .. 4 t + 3
-#pragma unroll 2
+#pragma unroll 4
                 for (int c4 = 0; c4 < RP / 4; ++c4) {
                     float pr[4];
 #pragma unroll
@@ -693,28 +713,9 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
         if (prm.resid && wr && t == 0) prm.resid[p] = (float)sqrt(rss / (double)L);
         // ---- uncertainty propagation (reading R3): J = H A_F' on my channels, sigma_i^2 = sum_l (J_il s_l)^2
         if (prm.coeff_sigma) {
-            float2 sv[NC / 2];
-            bool sbad = false;
-            if (prm.has_sigma) {
-                const float *sp = prm.sigma + p * prm.sigma_stride;
 #pragma unroll
-                for (int v = 0; v < LQ; ++v) {
-                    const int l = 4 * (t + 8 * v);
-                    float4 t4;
-                    if (svec_ok && l + 3 < L) {
-                        t4 = *reinterpret_cast<const float4 *>(sp + l);
-                    } else {
-                        t4.x = (l + 0 < L) ? sp[l + 0] : 1.0f; t4.y = (l + 1 < L) ? sp[l + 1] : 1.0f;
-                        t4.z = (l + 2 < L) ? sp[l + 2] : 1.0f; t4.w = (l + 3 < L) ? sp[l + 3] : 1.0f;
-                    }
-                    sv[2 * v] = make_float2(t4.x, t4.y); sv[2 * v + 1] = make_float2(t4.z, t4.w);
-                    sbad |= !(t4.x > 0.0f) || !isfinite(t4.x) || !(t4.y > 0.0f) || !isfinite(t4.y);
-                    sbad |= !(t4.z > 0.0f) || !isfinite(t4.z) || !(t4.w > 0.0f) || !isfinite(t4.w);
-                }
-            } else {
-#pragma unroll
-                for (int c = 0; c < NC / 2; ++c) sv[c] = make_float2(1.0f, 1.0f);
-            }
+            for (int c = 0; c < NC / 2; ++c)
+                sbad |= !(sv[c].x > 0.0f) || !isfinite(sv[c].x) || !(sv[c].y > 0.0f) || !isfinite(sv[c].y);
             sbad = ((__ballot_sync(FULL, sbad) >> (8 * g)) & 0xffu) != 0u;
             if (wr && sbad) info |= LINMIN_INFO_BAD_SIGMA;
             const bool doj = (st == 1) && !sbad && k > 1;
@@ -726,26 +727,30 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 for (int ii = 0; ii < IT; ++ii)
 #pragma unroll
                     for (int c = 0; c < NC / 2; ++c) d[ii][c] = make_float2(0.0f, 0.0f);
+                // branch-free body (a pixel whose support ends before j, or that has no J to form, multiplies
+                // by zero): the loads of step j + 1 can be issued under the FFMA2 stream of step j
+#pragma unroll 2
                 for (int j = 0; j < kj; ++j) {
-                    if (doj && j < k && ib < k) {
-                        float hh[IT];
-                        if (IT == 4) {
-                            const float4 h4 = *reinterpret_cast<const float4 *>(Hs + j * 16 + ib);
-                            hh[0] = h4.x; hh[1] = h4.y; hh[IT - 2] = h4.z; hh[IT - 1] = h4.w;
-                        } else {
-                            const float2 h2 = *reinterpret_cast<const float2 *>(Hs + j * 16 + ib);
-                            hh[0] = h2.x; hh[1] = h2.y;
-                        }
-                        const float *row = At32 + (size_t)idx[j] * RS + 4 * t;
+                    const bool on = doj && j < k && ib < k;
+                    float hh[IT];
+                    if (IT == 4) {
+                        const float4 h4 = *reinterpret_cast<const float4 *>(Hs + j * 16 + ib);
+                        hh[0] = h4.x; hh[1] = h4.y; hh[IT - 2] = h4.z; hh[IT - 1] = h4.w;
+                    } else {
+                        const float2 h2 = *reinterpret_cast<const float2 *>(Hs + j * 16 + ib);
+                        hh[0] = h2.x; hh[1] = h2.y;
+                    }
 #pragma unroll
-                        for (int v = 0; v < LQ; ++v) {
-                            const float4 a4 = *reinterpret_cast<const float4 *>(row + 32 * v);
-                            const float2 alo = make_float2(a4.x, a4.y), ahi = make_float2(a4.z, a4.w);
+                    for (int ii = 0; ii < IT; ++ii) hh[ii] = on ? hh[ii] : 0.0f;
+                    const float *row = At32 + (size_t)idx[j] * RS + 4 * t;
 #pragma unroll
-                            for (int ii = 0; ii < IT; ++ii) {
-                                d[ii][2 * v] = fma2(hh[ii], alo, d[ii][2 * v]);
-                                d[ii][2 * v + 1] = fma2(hh[ii], ahi, d[ii][2 * v + 1]);
-                            }
+                    for (int v = 0; v < LQ; ++v) {
+                        const float4 a4 = *reinterpret_cast<const float4 *>(row + 32 * v);
+                        const float2 alo = make_float2(a4.x, a4.y), ahi = make_float2(a4.z, a4.w);
+#pragma unroll
+                        for (int ii = 0; ii < IT; ++ii) {
+                            d[ii][2 * v] = fma2(hh[ii], alo, d[ii][2 * v]);
+                            d[ii][2 * v + 1] = fma2(hh[ii], ahi, d[ii][2 * v + 1]);
                         }
                     }
                 }
@@ -792,14 +797,13 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
     }
 }
 
-inline bool finish_sweep_supported(int L, int R) { return R <= 32 && L <= 256; }
 
 template <int LQ>
 inline cudaError_t launch_finish_sweep_lq(const LibView &lv, const SolveParams &prm, int sm_count,
                                           unsigned int *counter, unsigned int *overflow, cudaStream_t stream) {
     const size_t cta = (fs::cta_bytes(LQ) + 15) & ~(size_t)15;
     const size_t per_warp = 4 * (size_t)fs::PIX_BYTES + 128;     // scratch of 4 pixels + the chunk permutation
-    int warps = (int)std::min<size_t>(13, (227 * 1024 - cta) / per_warp);
+    int warps = (int)std::min<size_t>(12, (227 * 1024 - cta) / per_warp);
     if (warps < 1) return cudaErrorInvalidConfiguration;
     const size_t smem = cta + per_warp * warps;
     cudaError_t e = cudaFuncSetAttribute(finish_sweep_kernel<LQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -12,14 +12,19 @@
 
 #include "common.cuh"
 #include "finish.cuh"
-#include "finish8.cuh"
 #include "finish_fast.cuh"
-#include "finish_sweep.cuh"
 #include "ipls_generic.cuh"
 #include "ipls_r32.cuh"
 #include "precompute.cuh"
 
 using namespace linmin;
+
+namespace linmin {
+// finish_sweep.cu (own translation unit, own register budget)
+cudaError_t launch_finish_sweep_tu(const LibView &lv, const SolveParams &prm, int sm_count,
+                                   unsigned int *counter, unsigned int *overflow, cudaStream_t stream);
+inline bool finish_sweep_supported(int L, int R) { return R <= 32 && L <= 256; }
+}  // namespace linmin
 
 struct linmin_library {
     int L = 0, R = 0;
@@ -131,8 +136,8 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
 
     // ---- K1: projection + IPLS
     // per-call workspace, because one handle may serve several streams: three work counters of the
-    // persistent kernels, then the overflow list of finish8 (count + one entry per pixel)
-    const bool use_f8 = finish8_supported(L, R);
+    // persistent kernels, then the overflow list of finish_sweep (count + one entry per pixel)
+    const bool use_f8 = finish_sweep_supported(L, R);
     unsigned int *ws = nullptr;
     const size_t ws_words = 4 + (use_f8 ? (size_t)N + 1 : 0);
     CK(cudaMallocAsync((void **)&ws, ws_words * sizeof(unsigned int), o.stream));
@@ -162,9 +167,9 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     if (lib->timing) CK(cudaEventRecord(lib->ev[1], o.stream));
     // ---- K2: exact finish + uncertainty + residual
     if (use_f8) {
-        CK(launch_finish_sweep(lv, prm, lib->sm_count, counters + 1, overflow, o.stream));
+        CK(launch_finish_sweep_tu(lv, prm, lib->sm_count, counters + 1, overflow, o.stream));
         ++launches;
-        // pixels whose support outgrew finish8 (none on the synthetic cubes): one-warp-per-pixel kernel
+        // pixels whose support outgrew finish_sweep (none on the synthetic cubes): one-warp-per-pixel kernel
         CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, o.stream));
         ++launches;
     } else if (finish_fast_supported(L, R)) {

@@ -181,7 +181,7 @@ def test_degenerate_inputs(lm):
 
 
 def test_large_supports_take_the_overflow_path(lm):
-    """Supports beyond finish8's cap (16 members) are finished by the one-warp-per-pixel kernel:
+    """Supports beyond finish_sweep's cap (16 members) are finished by the one-warp-per-pixel kernel:
     dense abundances on a well-conditioned random library, mixed with sparse pixels."""
     import oracle
     from parity import check_parity
