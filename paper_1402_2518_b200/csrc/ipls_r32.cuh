@@ -493,40 +493,37 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                         else m2[s][k1 >> 1].x = fmaf(nl[s], ck1, m2[s][k1 >> 1].x);
                     }
                 }
-                float4 n4[8];
-                float2 zn = make_float2(0.0f, 0.0f);
+                const float *cb = (k1 & 1) ? xb1 : xb0;
                 if (k1 < 31) {
-                    float *cb = (k1 & 1) ? xb1 : xb0;
+                    float *cw = (k1 & 1) ? xb1 : xb0;
 #pragma unroll
-                    for (int s = s1; s < 4; ++s) cb[t + 8 * s] = LM_COL(s, k1);
-                    *reinterpret_cast<float2 *>(cb + 32 + 2 * t) = rr[s1];
+                    for (int s = s1; s < 4; ++s) cw[t + 8 * s] = LM_COL(s, k1);
+                    *reinterpret_cast<float2 *>(cw + 32 + 2 * t) = rr[s1];
                     __syncwarp();
-                    zn = *reinterpret_cast<const float2 *>(cb + 32 + 2 * (k1 & 7));
-#pragma unroll
-                    for (int c = k1 >> 2; c < 8; ++c) n4[c] = *reinterpret_cast<const float4 *>(cb + 4 * c);
+                    zk = *reinterpret_cast<const float2 *>(cb + 32 + 2 * (k1 & 7));
                 }
-                // ---- rest of the rank-one update of step k: columns k + 2 ..
+                // ---- rest of the rank-one update of step k (columns k + 2 ..), chunk by chunk; a chunk of
+                //      column k is replaced by the same chunk of column k + 1 as soon as it has been used
+                //      (one column buffer in registers; the pivot chunk is reloaded first)
 #pragma unroll
-                for (int c = (k + 2) >> 2; c < 8; ++c) {
+                for (int c = k1 >> 2; c < 8; ++c) {
+                    if (c >= ((k + 2) >> 2)) {
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const int jp = 2 * c + h, j0 = 2 * jp;
-                        const float2 cp = h ? make_float2(l4[c].z, l4[c].w) : make_float2(l4[c].x, l4[c].y);
-                        if (j0 >= k + 2) {
+                        for (int h = 0; h < 2; ++h) {
+                            const int jp = 2 * c + h, j0 = 2 * jp;
+                            const float2 cp = h ? make_float2(l4[c].z, l4[c].w) : make_float2(l4[c].x, l4[c].y);
+                            if (j0 >= k + 2) {
 #pragma unroll
-                            for (int s = s0; s < 4; ++s)
-                                if (j0 < 8 * s + 8) m2[s][jp] = fma2(nl[s], cp, m2[s][jp]);
-                        } else if (j0 + 1 == k + 2) {
+                                for (int s = s0; s < 4; ++s)
+                                    if (j0 < 8 * s + 8) m2[s][jp] = fma2(nl[s], cp, m2[s][jp]);
+                            } else if (j0 + 1 == k + 2) {
 #pragma unroll
-                            for (int s = s0; s < 4; ++s)
-                                if (j0 < 8 * s + 8) m2[s][jp].y = fmaf(nl[s], cp.y, m2[s][jp].y);
+                                for (int s = s0; s < 4; ++s)
+                                    if (j0 < 8 * s + 8) m2[s][jp].y = fmaf(nl[s], cp.y, m2[s][jp].y);
+                            }
                         }
                     }
-                }
-                if (k1 < 31) {
-                    zk = zn;
-#pragma unroll
-                    for (int c = k1 >> 2; c < 8; ++c) l4[c] = n4[c];
+                    if (k1 < 31) l4[c] = *reinterpret_cast<const float4 *>(cb + 4 * c);
                 }
             }
 #undef L4C
