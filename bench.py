@@ -29,6 +29,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_1402_2518_b200.shard import cube_block, max_over_ranks  # noqa: E402
 from paper_1402_2518_b200.synth import CONFIGS, make_cube, make_library  # noqa: E402
 
 METRIC = "unmixed spectra/sec"
@@ -196,7 +197,7 @@ def main():
     t_gen = time.perf_counter()
     Yh = torch.empty((N, L), dtype=torch.float32, pin_memory=True)
     Sh = torch.empty((N, L), dtype=torch.float32, pin_memory=True)
-    A = gen_cubes(rank * n_cubes, n_cubes, Yh.numpy(), Sh.numpy(), threads)
+    A = gen_cubes(cube_block(rank, n_cubes)[0], n_cubes, Yh.numpy(), Sh.numpy(), threads)
     t_gen = time.perf_counter() - t_gen
     Ad = torch.from_numpy(A).to(dev)
     Yd = Yh.to(dev, non_blocking=True)
@@ -237,10 +238,7 @@ def main():
     clocks = sampler.stop()
     ms_total = ev0.elapsed_time(ev1)
     ms_step = ms_total / args.steps
-    if world > 1:
-        t = torch.tensor([ms_step], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step = float(t.item())
+    ms_step = max_over_ranks(ms_step, dev)
     value = world * N / (ms_step * 1e-3)
     launches = lib.last_launches() * args.steps
 
@@ -317,10 +315,7 @@ def main():
             linmin.unmix_host(Ah, Yh, Sh, out=hout)
         barrier()
         dt = (time.perf_counter() - t0) / args.e2e_steps
-        if world > 1:
-            t = torch.tensor([dt], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, dev)
         e2e = {"value": world * N / dt, "unit": UNIT, "h2d_bytes_per_step": int(2 * N * L * 4 + L * R * 4),
                "d2h_bytes_per_step": int(N * (2 * R + 1) * 4), "ms_per_step": dt * 1e3, "steps": args.e2e_steps,
                "api": "linmin_unmix_host (pinned host buffers, 3-deep chunk pipeline)"}
