@@ -19,7 +19,7 @@
 //   * The forward substitution of the predictor (right-hand sides 1 and -w) is fused into the
 //     factorisation: the two right-hand sides ride along as a packed pair per row.
 //   * Blocked substitutions: every lane forms its row of the inverse of the four 8 x 8 diagonal blocks
-//     of L; a substitution is then 7 exchanges through shared memory (all-gather in the forward,
+//     of L (under the FFMA2 stream of the factorisation, as soon as a block is final); a substitution is then 7 exchanges through shared memory (all-gather in the forward,
 //     reduce-scatter in the backward direction) instead of a 31-step shuffle chain.
 //   * G, Gi (padded rows), the centred library (re-laid out so that a lane's four rows are one LDS.128)
 //     and the channel means live in shared memory, loaded once per CTA; warps run independently on
@@ -450,6 +450,36 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             float2 rr[4];
 #pragma unroll
             for (int s = 0; s < 4; ++s) rr[s] = make_float2(1.0f, -w[s]);
+            // Diagonal blocks of -L go to shared memory as soon as they are final, and every lane forms its row
+            // of T_s^-1 (x_j = [j == t] + sum_{i > j} x_i (-L)_{i j}) two steps later, under the FFMA2 stream of
+            // the factorisation instead of in a latency-bound phase of its own.
+            float2 ti[4][4];
+#define TINV_STORE(s_)                                                                                          \
+    {                                                                                                           \
+        *reinterpret_cast<float4 *>(Tb + (s_) * 64 + t * 8) =                                                   \
+            make_float4(m2[s_][4 * (s_)].x, m2[s_][4 * (s_)].y, m2[s_][4 * (s_) + 1].x, m2[s_][4 * (s_) + 1].y); \
+        *reinterpret_cast<float4 *>(Tb + (s_) * 64 + t * 8 + 4) = make_float4(                                  \
+            m2[s_][4 * (s_) + 2].x, m2[s_][4 * (s_) + 2].y, m2[s_][4 * (s_) + 3].x, m2[s_][4 * (s_) + 3].y);    \
+    }
+#define TINV_ROWS(s_)                                                                            \
+    {                                                                                            \
+        float T[8][8];                                                                           \
+        _Pragma("unroll") for (int i = 1; i < 8; ++i) {                                          \
+            const float4 u = *reinterpret_cast<const float4 *>(Tb + (s_) * 64 + i * 8);          \
+            T[i][0] = u.x; T[i][1] = u.y; T[i][2] = u.z; T[i][3] = u.w;                          \
+            if (i > 4) {                                                                         \
+                const float4 v = *reinterpret_cast<const float4 *>(Tb + (s_) * 64 + i * 8 + 4);  \
+                T[i][4] = v.x; T[i][5] = v.y; T[i][6] = v.z; T[i][7] = v.w;                      \
+            }                                                                                    \
+        }                                                                                        \
+        float x[8];                                                                              \
+        _Pragma("unroll") for (int j = 7; j >= 0; --j) {                                         \
+            float v = (t == j) ? 1.0f : 0.0f;                                                    \
+            _Pragma("unroll") for (int i = j + 1; i < 8; ++i) v = fmaf(x[i], T[i][j], v);        \
+            x[j] = v;                                                                            \
+        }                                                                                        \
+        _Pragma("unroll") for (int jp = 0; jp < 4; ++jp) ti[s_][jp] = make_float2(x[2 * jp], x[2 * jp + 1]); \
+    }
             bool clamped = false;
             // Look-ahead schedule: column k + 1 is updated and put on the exchange line BEFORE the rest of
             // the rank-one update of step k, so that the shared-memory round trip of step k + 1 overlaps
@@ -470,6 +500,12 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             for (int k = 0; k < 31; ++k) {
                 const int s0 = k >> 3, t0 = k & 7;
                 const int k1 = k + 1, s1 = k1 >> 3;
+                if (k == 7) TINV_STORE(0)
+                if (k == 15) TINV_STORE(1)
+                if (k == 23) TINV_STORE(2)
+                if (k == 9) TINV_ROWS(0)
+                if (k == 17) TINV_ROWS(1)
+                if (k == 25) TINV_ROWS(2)
                 float piv = L4C(k);
                 if (!(piv > pivot_floor)) { piv = pivot_floor; clamped = true; }
                 const float rinv = rcp_approx(piv);
@@ -535,40 +571,12 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                 m2[3][15].y = 0.0f;
             }
             if (__any_sync(0xffu << (8 * g), clamped)) flags |= LINMIN_INFO_CHOL_REGULARISED;
-            // ---- diagonal blocks of -L to shared memory; every lane forms its row of T_s^-1:
-            //      x_j = [j == t] + sum_{i > j} x_i (-L)_{i j}  (row t of the inverse of a unit lower matrix)
-#pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                *reinterpret_cast<float4 *>(Tb + s * 64 + t * 8) =
-                    make_float4(m2[s][4 * s].x, m2[s][4 * s].y, m2[s][4 * s + 1].x, m2[s][4 * s + 1].y);
-                *reinterpret_cast<float4 *>(Tb + s * 64 + t * 8 + 4) =
-                    make_float4(m2[s][4 * s + 2].x, m2[s][4 * s + 2].y, m2[s][4 * s + 3].x, m2[s][4 * s + 3].y);
-            }
+            // ---- last diagonal block (blocks 0..2 were inverted under the factorisation)
+            TINV_STORE(3)
             __syncwarp();
-            float2 ti[4][4];
-#pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                float T[8][8];
-#pragma unroll
-                for (int i = 1; i < 8; ++i) {
-                    const float4 u = *reinterpret_cast<const float4 *>(Tb + s * 64 + i * 8);
-                    T[i][0] = u.x; T[i][1] = u.y; T[i][2] = u.z; T[i][3] = u.w;
-                    if (i > 4) {
-                        const float4 v = *reinterpret_cast<const float4 *>(Tb + s * 64 + i * 8 + 4);
-                        T[i][4] = v.x; T[i][5] = v.y; T[i][6] = v.z; T[i][7] = v.w;
-                    }
-                }
-                float x[8];
-#pragma unroll
-                for (int j = 7; j >= 0; --j) {
-                    float v = (t == j) ? 1.0f : 0.0f;
-#pragma unroll
-                    for (int i = j + 1; i < 8; ++i) v = fmaf(x[i], T[i][j], v);
-                    x[j] = v;
-                }
-#pragma unroll
-                for (int jp = 0; jp < 4; ++jp) ti[s][jp] = make_float2(x[2 * jp], x[2 * jp + 1]);
-            }
+            TINV_ROWS(3)
+#undef TINV_STORE
+#undef TINV_ROWS
             PH(3)
             // ---- predictor: M^-1 = L^-T D^-1 L^-1; nu eliminated through L^-1 1
             float sww = 0.0f, swz = 0.0f;
