@@ -489,9 +489,8 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             {
 #pragma unroll
                 for (int s = 0; s < 4; ++s) xb0[t + 8 * s] = LM_COL(s, 0);
-                *reinterpret_cast<float2 *>(xb0 + 32 + 2 * t) = rr[0];
                 __syncwarp();
-                zk = *reinterpret_cast<const float2 *>(xb0 + 32);
+                zk = make_float2(__shfl_sync(FULL, rr[0].x, 0, 8), __shfl_sync(FULL, rr[0].y, 0, 8));
 #pragma unroll
                 for (int c = 0; c < 8; ++c) l4[c] = *reinterpret_cast<const float4 *>(xb0 + 4 * c);
             }
@@ -534,9 +533,10 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                     float *cw = (k1 & 1) ? xb1 : xb0;
 #pragma unroll
                     for (int s = s1; s < 4; ++s) cw[t + 8 * s] = LM_COL(s, k1);
-                    *reinterpret_cast<float2 *>(cw + 32 + 2 * t) = rr[s1];
                     __syncwarp();
-                    zk = *reinterpret_cast<const float2 *>(cb + 32 + 2 * (k1 & 7));
+                    // right-hand sides of row k + 1: two shuffles (off the pivot chain) instead of a store and
+                    // a load on the shared-memory pipe, which is the busiest unit of this kernel
+                    zk = make_float2(__shfl_sync(FULL, rr[s1].x, k1 & 7, 8), __shfl_sync(FULL, rr[s1].y, k1 & 7, 8));
                 }
                 // ---- rest of the rank-one update of step k (columns k + 2 ..), chunk by chunk; a chunk of
                 //      column k is replaced by the same chunk of column k + 1 as soon as it has been used
