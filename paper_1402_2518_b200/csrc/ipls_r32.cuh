@@ -101,7 +101,7 @@ __device__ __forceinline__ float gmax(float v) {
 // shared-memory footprint in floats
 __host__ __device__ inline int lpad(int L) { return (L + 3) & ~3; }
 __host__ __device__ inline size_t smem_floats(int L) {
-    return (size_t)2 * R * GST + 2 * R         // Gp, Gip, row sums of Gi (and their total)
+    return (size_t)2 * R * GST + 3 * R         // Gp, Gip, row sums of Gi (and their total), row sums of G
            + (size_t)lpad(L) * R + lpad(L)      // Acp, c
            + (size_t)WARPS * 4 * (PIXF + 2 * lpad(L));
 }
@@ -191,7 +191,8 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
     float *Gp = smem;                        // [32][GST]
     float *Gip = Gp + R * GST;               // [32][GST] inverse of the regularised G (start point)
     float *Giq = Gip + R * GST;              // [32] row sums of Gi, [32] their total
-    float *Acp = Giq + 2 * R;                // [Lp][32]: Acp[l][t*4+s] = Ac[l][t+8s]
+    float *Grs = Giq + 2 * R;                // [32] row sums of G
+    float *Acp = Grs + R;                    // [Lp][32]: Acp[l][t*4+s] = Ac[l][t+8s]
     float *cv = Acp + (size_t)Lp * R;        // [Lp]
     const int lane = threadIdx.x & 31, g = lane >> 3, t = lane & 7;
     float *pix = cv + Lp + (size_t)((threadIdx.x >> 5) * 4 + g) * (PIXF + 2 * Lp);
@@ -220,6 +221,11 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         float s = 0.0f;
         for (int j = 0; j < R; ++j) s += Giq[j];
         Giq[R] = s;
+    }
+    if (threadIdx.x >= 32 && threadIdx.x < 32 + R) {
+        float s = 0.0f;
+        for (int j = 0; j < R; ++j) s += Gp[(threadIdx.x - 32) * GST + j];
+        Grs[threadIdx.x - 32] = s;
     }
     __syncthreads();
 
@@ -306,7 +312,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
 
         // ---- start (Mehrotra's heuristic on this QP): x = the sum-constrained LS point of the regularised
         //      problem, lambda = its reduced gradient, both shifted into the interior
-        float a[4], lam[4], w[4];
+        float a[4], lam[4], w[4], Ga[4];
         float nu, lam0;
         {
             __syncwarp();
@@ -349,7 +355,8 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             float gx = 0.0f, mnx = INFINITY, mng = INFINITY;
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
-                lam[s] = x2[s].x + x2[s].y - b[s];          // gradient at x
+                Ga[s] = x2[s].x + x2[s].y;                  // G x
+                lam[s] = Ga[s] - b[s];                      // gradient at x
                 gx = fmaf(lam[s], x[s], gx);
                 mnx = fminf(mnx, x[s]); mng = fminf(mng, lam[s]);
             }
@@ -374,11 +381,14 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             sa = gsum(sa); lam0 = gmax(lm);
             const float rsa = 1.0f / sa;
 #pragma unroll
-            for (int s = 0; s < 4; ++s) a[s] *= rsa;
+            for (int s = 0; s < 4; ++s) {
+                a[s] *= rsa;
+                Ga[s] = fmaf(dp + dp2 + 1e-3f, Grs[t + 8 * s], Ga[s]) * rsa;     // G a of the shifted, normalised point
+            }
             if (!(lam0 > 0.0f) || !isfinite(lam0) || !isfinite(sa)) {     // degenerate data: fall back to the flat start
                 lam0 = fmaxf(bmax, 1e-3f * gdmax);
 #pragma unroll
-                for (int s = 0; s < 4; ++s) { a[s] = 1.0f / 32.0f; lam[s] = lam0; }
+                for (int s = 0; s < 4; ++s) { a[s] = 1.0f / 32.0f; lam[s] = lam0; Ga[s] = Grs[t + 8 * s] * (1.0f / 32.0f); }
                 nu = 0.0f;
             }
         }
@@ -387,27 +397,17 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
 
         PH(7)
         for (int it = 0;; ++it) {
-            // ---- exchange a (line 1: step 0 of the factorisation writes line 0); G a and M rows
-            __syncwarp();
-#pragma unroll
-            for (int s = 0; s < 4; ++s) xb1[t + 8 * s] = a[s];
-            __syncwarp();
+            // ---- rows of M (lower part) from G.  G a is not recomputed: the Newton system gives
+            //      G da = (r1 - dnu 1) - d o da row by row, so G a is carried along with a (no exchange of a,
+            //      no loads of the upper part of G: 80 wavefronts less on the shared-memory pipe per iteration)
             float2 m2[4][16];
-            float2 Ga2[4];
 #pragma unroll
-            for (int s = 0; s < 4; ++s) Ga2[s] = make_float2(0.0f, 0.0f);
+            for (int s = 0; s < 4; ++s) {
 #pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                const float4 a4 = *reinterpret_cast<const float4 *>(xb1 + 4 * c);
-#pragma unroll
-                for (int s = 0; s < 4; ++s) {
+                for (int c = 0; c < 2 * s + 2; ++c) {
                     const float4 g4 = *reinterpret_cast<const float4 *>(Gp + (t + 8 * s) * GST + 4 * c);
-                    Ga2[s] = fma2(make_float2(g4.x, g4.y), make_float2(a4.x, a4.y), Ga2[s]);
-                    Ga2[s] = fma2(make_float2(g4.z, g4.w), make_float2(a4.z, a4.w), Ga2[s]);
-                    if (4 * c < 8 * s + 8) {
-                        m2[s][2 * c] = make_float2(g4.x, g4.y);
-                        m2[s][2 * c + 1] = make_float2(g4.z, g4.w);
-                    }
+                    m2[s][2 * c] = make_float2(g4.x, g4.y);
+                    m2[s][2 * c + 1] = make_float2(g4.z, g4.w);
                 }
             }
             PH(0)
@@ -415,7 +415,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             float rdm = 0.0f, sa = 0.0f, gp = 0.0f;
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
-                w[s] = Ga2[s].x + Ga2[s].y - b[s] + nu;
+                w[s] = Ga[s] - b[s] + nu;
                 rdm = fmaxf(rdm, fabsf(w[s] - lam[s]));
                 sa += a[s];
                 gp = fmaf(a[s], lam[s], gp);
@@ -640,6 +640,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             if (done) { ap = 0.0f; ad = 0.0f; }                // converged pixels ride along unchanged
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
+                Ga[s] = fmaf(ap, fmaf(cc[s], ainv[s], -w[s]) - dnu - d[s] * da[s], Ga[s]);
                 a[s] = fmaxf(fmaf(ap, da[s], a[s]), 1e-18f);
                 lam[s] = fmaxf(fmaf(ad, dl[s], lam[s]), 1e-18f * lam0);
             }
