@@ -13,7 +13,8 @@
 //
 // This generic kernel keeps everything of a pixel in shared memory and lets a TEAM of threads
 // (a warp, or the whole CTA for R > 64) cooperate on the Cholesky factorisation and the triangular
-// solves.  It is the any-size reference path; R = 32 has a register-blocked kernel of its own.
+// solves.  It is the any-size path; R = 32 has a register-blocked kernel of its own.  Like that kernel it
+// starts from Mehrotra's heuristic point and carries G a along with a (no mat-vec per iteration).
 #pragma once
 #include "common.cuh"
 
@@ -61,8 +62,9 @@ struct TeamOps {
 };
 
 // In-place left-looking Cholesky of the packed (column-major lower) n x n matrix Mp.
-// dinv[j] = 1/L_jj; the diagonal of Mp keeps the ORIGINAL M_jj (every thread re-derives the pivot
-// from it, so it must not be overwritten while the column is in flight; L_jj = 1/dinv[j]).
+// dinv[j] = 1/L_jj.  The diagonal slot of row i carries the running pivot M_ii - sum_{k<j} L_ik^2: the
+// thread that finishes L_ij subtracts its square at once, so the pivot of column j is ONE load for every
+// thread instead of a j-term recomputation (that loop was half of the kernel's work).
 // A pivot below `floorv` is clamped (returns true if that happened).
 template <int TEAM, typename T>
 __device__ __forceinline__ bool team_cholesky(T *Mp, T *dinv, int n, T floorv) {
@@ -71,19 +73,46 @@ __device__ __forceinline__ bool team_cholesky(T *Mp, T *dinv, int n, T floorv) {
     bool clamped = false;
     for (int j = 0; j < n; ++j) {
         T sj = Mp[cm(n, j, j)];
-        for (int k = 0; k < j; ++k) {
-            T ljk = Mp[cm(n, j, k)];
-            sj -= ljk * ljk;
-        }
         if (!(sj > floorv)) { sj = floorv; clamped = true; }
-        T dj = (T)1 / sqrt(sj);
-        for (int i = j + t; i < n; i += TEAM) {
-            if (i == j) {
-                dinv[j] = dj;
-            } else {
-                T s = Mp[cm(n, i, j)];
-                for (int k = 0; k < j; ++k) s -= Mp[cm(n, i, k)] * Mp[cm(n, j, k)];
-                Mp[cm(n, i, j)] = s * dj;
+        const T dj = (T)1 / sqrt(sj);
+        if (t == 0) dinv[j] = dj;
+        // Rows j+1 .. n-1 of column j: L_ij = (M_ij - sum_{k<j} L_ik L_jk) / L_jj.  When fewer rows than
+        // threads remain, g = 2, 4, .. 32 lanes (of one warp) share a row: each takes every g-th term of the
+        // sum and the parts are added by shuffles, so the late columns (long sums, few rows) keep the whole
+        // team busy instead of leaving most of it at the barrier.
+        const int nr = n - 1 - j;
+        int g = 1;
+        while (g < 32 && nr * (g * 2) <= TEAM) g <<= 1;
+        const int rows_per_pass = TEAM / g;
+        const int part = t & (g - 1), rl = t / g;
+        for (int r0 = 0; r0 < nr; r0 += rows_per_pass) {
+            const int i = j + 1 + r0 + rl;
+            const bool active = i < n;
+            const int ii = active ? i : j;                      // a valid row for the loads of idle lanes
+            // element (r, k) of the packed matrix sits at cb(k) + r with cb(k) = k (n - 1) - k (k - 1)/2
+            // my terms k = part, part + g, ..: cb advances by d, d shrinks by g^2 (no multiply in the loop);
+            // four partial sums keep four load pairs in flight
+            T s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+            int k = part;
+            int c = k * (n - 1) - ((k * (k - 1)) >> 1);
+            int d = g * (n - 1) - ((g * (g - 1)) >> 1) - g * k;
+            const int g2 = g * g;
+            for (; k + 3 * g < j; k += 4 * g) {
+                const int c0 = c, c1 = c0 + d, c2 = c1 + d - g2, c3 = c2 + d - 2 * g2;
+                s0 += Mp[c0 + ii] * Mp[c0 + j];
+                s1 += Mp[c1 + ii] * Mp[c1 + j];
+                s2 += Mp[c2 + ii] * Mp[c2 + j];
+                s3 += Mp[c3 + ii] * Mp[c3 + j];
+                c = c3 + d - 3 * g2;
+                d -= 4 * g2;
+            }
+            for (; k < j; k += g) { s0 += Mp[c + ii] * Mp[c + j]; c += d; d -= g2; }
+            T s = (s0 + s1) + (s2 + s3);
+            for (int o = g >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (active && part == 0) {
+                s = (Mp[cm(n, i, j)] - s) * dj;
+                Mp[cm(n, i, j)] = s;
+                Mp[cm(n, i, i)] -= s * s;
             }
         }
         Ops::sync();
@@ -129,7 +158,7 @@ __device__ __forceinline__ void team_solve(const T *Mp, const T *dinv, int n, T 
 }
 
 __host__ __device__ inline size_t ipls_generic_team_floats(int L, int R) {
-    return (size_t)9 * R + L + (size_t)R * (R + 1) / 2 + 64;
+    return (size_t)10 * R + L + (size_t)R * (R + 1) / 2 + 64;
 }
 
 // grid-stride over pixels; TEAM == 32: one warp per pixel, blockDim.x/32 pixels per CTA pass;
@@ -144,7 +173,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
     const int t = Ops::tid();
     float *base = smem + (size_t)team * ipls_generic_team_floats(L, R);
     float *a = base, *lam = a + R, *b = lam + R, *w = b + R, *u = w + R, *v = u + R, *da = v + R,
-          *dl = da + R, *dinv = dl + R, *yc = dinv + R, *red = yc + L, *Mp = red + 64;
+          *dl = da + R, *dinv = dl + R, *Ga = dinv + R, *yc = Ga + R, *red = yc + L, *Mp = red + 64;
     const float fR = (float)R;
     const float tau = 0.995f;
 
@@ -173,22 +202,64 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
             for (int l = 0; l < L; ++l) s = fmaf(lib.Ac[(size_t)l * R + i], yc[l], s);
             b[i] = s;
             bmax = fmaxf(bmax, fabsf(s));
-            a[i] = 1.0f / fR;
         }
         bmax = Ops::max(bmax, red);
         const float sc = fmaxf(bmax, 1e-3f * lib.gdmax);
-        // start: a = 1/R, nu = 0, lambda = max(||G a - b||_inf, 1e-3 gdmax)
-        float g0 = 0.0f;
-        Ops::sync();
-        for (int i = t; i < R; i += TEAM) {
-            float s = 0.0f;
-            for (int j = 0; j < R; ++j) s = fmaf(lib.Gc[(size_t)j * R + i], a[j], s);
-            g0 = fmaxf(g0, fabsf(s - b[i]));
+        // ---- start (Mehrotra's heuristic, as in ipls_r32.cuh): the sum-constrained LS point of the regularised
+        //      problem, x = Gi b - q (1'Gi b - 1)/(1'q), its reduced gradient as multipliers, both shifted inside
+        float nu, lam0;
+        {
+            Ops::sync();
+            float sx = 0.0f, sq = 0.0f;
+            for (int i = t; i < R; i += TEAM) {
+                float s = 0.0f;
+                for (int j = 0; j < R; ++j) s = fmaf(lib.Gi[(size_t)j * R + i], b[j], s);
+                u[i] = s; sx += s; sq += lib.Giq[i];
+            }
+            sx = Ops::sum(sx, red); sq = Ops::sum(sq, red);
+            const float mu0 = (sx - 1.0f) / sq;
+            for (int i = t; i < R; i += TEAM) u[i] = fmaf(-mu0, lib.Giq[i], u[i]);       // x
+            Ops::sync();
+            float gx = 0.0f, mnx = INFINITY, mng = INFINITY;
+            for (int i = t; i < R; i += TEAM) {
+                float s = 0.0f, rs = 0.0f;
+                for (int j = 0; j < R; ++j) { const float gji = lib.Gc[(size_t)j * R + i]; s = fmaf(gji, u[j], s); rs += gji; }
+                Ga[i] = s;                    // G x
+                v[i] = rs;                    // row sum of G
+                const float gi = s - b[i];
+                lam[i] = gi;
+                gx = fmaf(gi, u[i], gx); mnx = fminf(mnx, u[i]); mng = fminf(mng, gi);
+            }
+            gx = Ops::sum(gx, red); mnx = Ops::min(mnx, red); mng = Ops::min(mng, red);
+            nu = -gx;
+            const float dp = fmaxf(-mnx, 0.0f), dd = fmaxf(-(mng + nu), 0.0f);
+            float xl = 0.0f, sl = 0.0f, sxx = 0.0f;
+            for (int i = t; i < R; i += TEAM) {
+                const float xi = u[i] + dp, li = lam[i] + nu + dd;
+                u[i] = xi; lam[i] = li;
+                xl = fmaf(xi, li, xl); sl += li; sxx += xi;
+            }
+            xl = Ops::sum(xl, red); sl = Ops::sum(sl, red); sxx = Ops::sum(sxx, red);
+            const float dp2 = 0.05f * xl / fmaxf(sl, 1e-30f), dd2 = 0.05f * xl / fmaxf(sxx, 1e-30f);
+            float sa = 0.0f, lm = 0.0f;
+            for (int i = t; i < R; i += TEAM) {
+                const float ai = u[i] + dp2 + 1e-3f, li = lam[i] + dd2 + 1e-4f * sc;
+                a[i] = ai; lam[i] = li;
+                sa += ai; lm = fmaxf(lm, li);
+            }
+            sa = Ops::sum(sa, red); lam0 = Ops::max(lm, red);
+            const float rsa = 1.0f / sa;
+            const bool ok = (lam0 > 0.0f) && isfinite(lam0) && isfinite(sa) && isfinite(rsa);
+            if (!ok) { lam0 = fmaxf(bmax, 1e-3f * lib.gdmax); nu = 0.0f; }
+            for (int i = t; i < R; i += TEAM) {
+                if (ok) {
+                    a[i] *= rsa;
+                    Ga[i] = fmaf(dp + dp2 + 1e-3f, v[i], Ga[i]) * rsa;      // G a of the shifted, normalised point
+                } else {                                                     // degenerate data: the barycentre
+                    a[i] = 1.0f / fR; lam[i] = lam0; Ga[i] = v[i] / fR;
+                }
+            }
         }
-        g0 = Ops::max(g0, red);
-        const float lam0 = fmaxf(g0, 1e-3f * lib.gdmax);
-        for (int i = t; i < R; i += TEAM) lam[i] = lam0;
-        float nu = 0.0f;
         int iters = 0, flags = 0;
         Ops::sync();
 
@@ -196,9 +267,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
             // ---- residuals
             float rdmax = 0.0f, suma = 0.0f, gap = 0.0f;
             for (int i = t; i < R; i += TEAM) {
-                float s = 0.0f;
-                for (int j = 0; j < R; ++j) s = fmaf(lib.Gc[(size_t)j * R + i], a[j], s);
-                float wi = s - b[i] + nu;
+                float wi = Ga[i] - b[i] + nu;      // G a is carried along with a (Newton identity, see the update)
                 w[i] = wi;
                 rdmax = fmaxf(rdmax, fabsf(wi - lam[i]));
                 suma += a[i];
@@ -270,7 +339,12 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
             }
             ap = fminf(1.0f, tau * Ops::min(ap, red));
             ad = fminf(1.0f, tau * Ops::min(ad, red));
+            // G da = (r1 - dnu 1) - (lambda/a) o da row by row (M da = r1 - dnu 1, M = G + diag(lambda/a)), with
+            // r1 = -w + cc/a and cc = dl + lambda + (lambda/a) da recovered from the corrector's dl
             for (int i = t; i < R; i += TEAM) {
+                const float di = lam[i] / a[i];
+                const float cc_over_a = dl[i] + lam[i] + di * da[i];
+                Ga[i] = fmaf(ap, (-w[i] + cc_over_a) - dnu - di * da[i], Ga[i]);
                 a[i] = fmaxf(fmaf(ap, da[i], a[i]), 1e-18f);
                 lam[i] = fmaxf(fmaf(ad, dl[i], lam[i]), 1e-18f * lam0);
             }
