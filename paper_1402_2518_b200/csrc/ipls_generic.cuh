@@ -125,6 +125,34 @@ template <int TEAM, int NRHS, typename T>
 __device__ __forceinline__ void team_solve(const T *Mp, const T *dinv, int n, T *x0, T *x1) {
     using Ops = TeamOps<TEAM>;
     const int t = Ops::tid();
+    if constexpr (TEAM == 32) {
+        // one warp, n <= 64: the right-hand sides live in registers (rows t and t + 32) and x_j travels by
+        // shuffle; a step is shuffle + FMA instead of store / barrier / load through shared memory
+        const int r1 = t + 32;
+        const bool h0 = t < n, h1 = r1 < n;
+        T a0 = h0 ? x0[t] : (T)0, b0 = h1 ? x0[r1] : (T)0;
+        T a1 = (NRHS > 1 && h0) ? x1[t] : (T)0, b1 = (NRHS > 1 && h1) ? x1[r1] : (T)0;
+        const T d0 = h0 ? dinv[t] : (T)0, d1 = h1 ? dinv[r1] : (T)0;
+        for (int j = 0; j < n; ++j) {      // forward: L z = rhs
+            const T dj = dinv[j];
+            const T z0 = __shfl_sync(0xffffffffu, (j < 32) ? a0 : b0, j & 31) * dj;
+            const T z1 = NRHS > 1 ? __shfl_sync(0xffffffffu, (j < 32) ? a1 : b1, j & 31) * dj : (T)0;
+            if (h0 && t > j) { const T l = Mp[cm(n, t, j)]; a0 -= l * z0; if (NRHS > 1) a1 -= l * z1; }
+            if (h1 && r1 > j) { const T l = Mp[cm(n, r1, j)]; b0 -= l * z0; if (NRHS > 1) b1 -= l * z1; }
+        }
+        a0 *= d0; b0 *= d1; a1 *= d0; b1 *= d1;
+        for (int j = n - 1; j >= 0; --j) { // backward: L' x = z
+            const T dj = dinv[j];
+            const T z0 = __shfl_sync(0xffffffffu, (j < 32) ? a0 : b0, j & 31) * dj;
+            const T z1 = NRHS > 1 ? __shfl_sync(0xffffffffu, (j < 32) ? a1 : b1, j & 31) * dj : (T)0;
+            if (t < j) { const T l = Mp[cm(n, j, t)]; a0 -= l * z0; if (NRHS > 1) a1 -= l * z1; }
+            if (r1 < j) { const T l = Mp[cm(n, j, r1)]; b0 -= l * z0; if (NRHS > 1) b1 -= l * z1; }
+        }
+        if (h0) { x0[t] = a0 * d0; if (NRHS > 1) x1[t] = a1 * d0; }
+        if (h1) { x0[r1] = b0 * d1; if (NRHS > 1) x1[r1] = b1 * d1; }
+        Ops::sync();
+        return;
+    }
     for (int j = 0; j < n; ++j) {          // forward: L z = rhs
         T z0 = x0[j] * dinv[j];
         T z1 = NRHS > 1 ? x1[j] * dinv[j] : (T)0;
