@@ -243,3 +243,26 @@ def test_odd_sizes(lm, L, R):
     g = run_gpu(lm, A, Y, sig)
     ora = oracle.solve(A, Y, sig)
     print(check_parity(A, Y, sig, g, ora, label=f"L{L}R{R}", require_unique=False))
+
+
+@pytest.mark.parametrize("name,N", [("omega", 40000), ("crism", 6000), ("tiny", 1000), ("stress", 900)])
+def test_results_do_not_depend_on_neighbours_or_repeats(lm, name, N):
+    """Stands in for racecheck (compute-sanitizer is closed on this pool): every pixel is an independent
+    problem, so its outputs must be bit-identical run to run, under a random permutation of
+    the pixels (other pixels share its warp, its 32-pixel chunk and its shared-memory scratch) and when it
+    is solved alone in a shorter batch.  A missing barrier or a read of another pixel's scratch breaks this."""
+    from paper_1402_2518_b200.synth import make_workload
+    w = make_workload(name, N=N)
+    g = run_gpu(lm, w.A, w.Y, w.sigma)
+    g2 = run_gpu(lm, w.A, w.Y, w.sigma)
+    rng = np.random.Generator(np.random.PCG64(7))
+    perm = rng.permutation(N)
+    gp = run_gpu(lm, w.A, np.ascontiguousarray(w.Y[perm]), np.ascontiguousarray(w.sigma[perm]))
+    m = 777 if N > 777 else N // 2
+    gs = run_gpu(lm, w.A, w.Y[:m], w.sigma[:m])
+    for key in ("coeffs", "coeff_sigma", "resid"):
+        assert np.array_equal(g[key], g2[key], equal_nan=True), f"{key}: run-to-run"
+        assert np.array_equal(g[key][perm], gp[key], equal_nan=True), f"{key}: permutation"
+        assert np.array_equal(g[key][:m], gs[key], equal_nan=True), f"{key}: shorter batch"
+    it, it_p = (g["info"] >> 8) & 0xff, (gp["info"] >> 8) & 0xff
+    assert np.array_equal(it[perm], it_p)
