@@ -151,8 +151,7 @@ __device__ __forceinline__ void team_solve(const T *Mp, const T *dinv, int n, T 
         if (h0) { x0[t] = a0 * d0; if (NRHS > 1) x1[t] = a1 * d0; }
         if (h1) { x0[r1] = b0 * d1; if (NRHS > 1) x1[r1] = b1 * d1; }
         Ops::sync();
-        return;
-    }
+    } else {
     for (int j = 0; j < n; ++j) {          // forward: L z = rhs
         T z0 = x0[j] * dinv[j];
         T z1 = NRHS > 1 ? x1[j] * dinv[j] : (T)0;
@@ -183,6 +182,7 @@ __device__ __forceinline__ void team_solve(const T *Mp, const T *dinv, int n, T 
         if (NRHS > 1) x1[i] *= dinv[i];
     }
     Ops::sync();
+    }
 }
 
 __host__ __device__ inline size_t ipls_generic_team_floats(int L, int R) {
