@@ -258,11 +258,17 @@ def main():
                 traffic = traffic * N
         except (OSError, ValueError):
             traffic = None
+    try:
+        ffma_tf, ffma2_tf = linmin.probe_fp32_peak()
+    except Exception:  # report helper only: never fail the bench line on it
+        ffma_tf, ffma2_tf = None, None
     roofline = {
         "bound": "alu", "kernel": "projection+IPLS kernel (K1)", "achieved": achieved,
         "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
         "traffic": traffic,
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no FP32 figure",
+        "peak_measured_TFLOPs": {"ffma": ffma_tf, "ffma2": ffma2_tf,
+                                 "how": "linmin_probe_fp32_peak: register-resident independent FMA chains, 8 CTAs x 256 threads per SM"},
         "kernel_ms": {"ipls": ipls_avg, "finish": fin_avg},
         "algorithmic_flops_per_pixel": {"ipls_kernel": f_ipls / N, "finish_kernel": f_fin / N},
         "whole_step": {"achieved": (f_ipls + f_fin) / (ms_step * 1e-3) / 1e12,

@@ -141,6 +141,12 @@ int linmin_library_last_launches(const linmin_library *lib);
 int linmin_library_enable_timing(linmin_library *lib, int enable);
 int linmin_library_last_timing(const linmin_library *lib, float *ipls_ms, float *finish_ms);
 
+/* Report helper for the roofline denominator (bench.py): measures what the FP32 FMA pipe of the current
+ * device sustains, in TFLOP/s (2 flops per FMA), with register-resident independent FMA chains: scalar
+ * FFMA in *ffma_tflops, packed FFMA2 (fma.rn.f32x2) in *ffma2_tflops (host pointers).  Synchronous; runs
+ * a few milliseconds of work on `stream` (a cudaStream_t, NULL = default stream).  Not on the hot path. */
+int linmin_probe_fp32_peak(void *stream, double *ffma_tflops, double *ffma2_tflops);
+
 const char *linmin_strerror(int code);
 int linmin_version(void);
 

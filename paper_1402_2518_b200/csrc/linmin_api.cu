@@ -16,6 +16,7 @@
 #include "ipls_generic.cuh"
 #include "ipls_r32.cuh"
 #include "precompute.cuh"
+#include "probe.cuh"
 
 using namespace linmin;
 
@@ -303,6 +304,15 @@ int linmin_debug_phases(unsigned long long *out16, int reset) {
 #endif
 
 int linmin_version(void) { return LINMIN_VERSION; }
+
+int linmin_probe_fp32_peak(void *stream, double *ffma_tflops, double *ffma2_tflops) {
+    if (!ffma_tflops || !ffma2_tflops) return LINMIN_ERR_INVALID_ARGUMENT;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(probe_fp32(sms, (cudaStream_t)stream, ffma_tflops, ffma2_tflops));
+    return LINMIN_OK;
+}
 
 const char *linmin_strerror(int code) {
     switch (code) {

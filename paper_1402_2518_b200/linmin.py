@@ -32,6 +32,7 @@ INFO_BAD_SIGMA = 0x20
 
 EXPORTS = ["linmin_version", "linmin_strerror", "linmin_library_create", "linmin_library_destroy",
            "linmin_library_last_launches", "linmin_library_enable_timing", "linmin_library_last_timing",
+           "linmin_probe_fp32_peak",
            "linmin_unmix_lib", "linmin_unmix", "linmin_unmix_host"]
 
 
@@ -71,6 +72,7 @@ def load() -> ctypes.CDLL:
         lib.linmin_library_last_launches.argtypes = [P]
         lib.linmin_library_enable_timing.argtypes = [P, ctypes.c_int]
         lib.linmin_library_last_timing.argtypes = [P, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]
+        lib.linmin_probe_fp32_peak.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
         lib.linmin_unmix_lib.argtypes = [P, P, P, I64, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_unmix.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_unmix_host.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
@@ -176,6 +178,13 @@ class Library:
             self.destroy()
         except Exception:
             pass
+
+
+def probe_fp32_peak(stream=None):
+    """(FFMA TFLOP/s, FFMA2 TFLOP/s) sustained by the FMA pipe of the current device (report helper)."""
+    a, b = ctypes.c_double(), ctypes.c_double()
+    _check(load().linmin_probe_fp32_peak(None if stream is None else ctypes.c_void_p(stream), ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
 
 
 def library_create(A) -> Library:
