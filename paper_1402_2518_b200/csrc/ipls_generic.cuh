@@ -185,6 +185,89 @@ __device__ __forceinline__ void team_solve(const T *Mp, const T *dinv, int n, T 
     }
 }
 
+// ---- warp-per-pixel path (R <= 64): the lower triangle of the Newton matrix is kept ROW-major, row i padded
+// to a multiple of 4 floats (16 B aligned rows; the footprint of the packed layout), so the sums of the
+// left-looking factorisation run over contiguous k: two LDS.128 feed four FMAs with no index arithmetic
+// (the packed column-major layout cost 30 instructions per four terms).
+// start of row i: rows 4b .. 4b+3 hold 4(b+1) floats each
+__host__ __device__ __forceinline__ int ipls_rowoff(int i) { const int b = i >> 2, r = i & 3; return 8 * b * (b + 1) + 4 * r * (b + 1); }
+__host__ __device__ inline int ipls_tri_floats(int n) { return n > 0 ? ipls_rowoff(n - 1) + 4 * (((n - 1) >> 2) + 1) : 0; }
+
+__device__ __forceinline__ bool warp_cholesky_rm(float *M, float *dinv, int n, float floorv) {
+    const int t = threadIdx.x & 31;
+    bool clamped = false;
+    for (int j = 0; j < n; ++j) {
+        float sj = M[ipls_rowoff(j) + j];               // running pivot (see team_cholesky)
+        if (!(sj > floorv)) { sj = floorv; clamped = true; }
+        const float dj = 1.0f / sqrtf(sj);
+        if (t == 0) dinv[j] = dj;
+        const int nr = n - 1 - j;
+        int g = 1;
+        while (g < 32 && nr * (g * 2) <= 32) g <<= 1;   // g lanes share one row when few rows remain
+        const int rows_per_pass = 32 / g;
+        const int part = t & (g - 1), rl = t / g;
+        const float *rowj = M + ipls_rowoff(j);
+        const int jv = j >> 2;                           // whole float4 chunks below column j
+        for (int r0 = 0; r0 < nr; r0 += rows_per_pass) {
+            const int i = j + 1 + r0 + rl;
+            const bool active = i < n;
+            float *rowi = M + ipls_rowoff(active ? i : j);
+            float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f, s3 = 0.0f;
+            for (int q = part; q < jv; q += g) {
+                const float4 a = *reinterpret_cast<const float4 *>(rowi + 4 * q);
+                const float4 b = *reinterpret_cast<const float4 *>(rowj + 4 * q);
+                s0 = fmaf(a.x, b.x, s0); s1 = fmaf(a.y, b.y, s1); s2 = fmaf(a.z, b.z, s2); s3 = fmaf(a.w, b.w, s3);
+            }
+            if (part == 0)
+                for (int k = 4 * jv; k < j; ++k) s0 = fmaf(rowi[k], rowj[k], s0);
+            float s = (s0 + s1) + (s2 + s3);
+            for (int o = g >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (active && part == 0) {
+                s = (rowi[j] - s) * dj;
+                rowi[j] = s;
+                rowi[i] -= s * s;
+            }
+        }
+        __syncwarp();
+    }
+    return clamped;
+}
+
+// (L L') x = rhs for the row-major factor: right-hand sides in registers (rows t, t + 32), x_j by shuffle
+template <int NRHS>
+__device__ __forceinline__ void warp_solve_rm(const float *M, const float *dinv, int n, float *x0, float *x1) {
+    const int t = threadIdx.x & 31, r1 = t + 32;
+    const bool h0 = t < n, h1 = r1 < n;
+    float a0 = h0 ? x0[t] : 0.0f, b0 = h1 ? x0[r1] : 0.0f;
+    float a1 = (NRHS > 1 && h0) ? x1[t] : 0.0f, b1 = (NRHS > 1 && h1) ? x1[r1] : 0.0f;
+    const float d0 = h0 ? dinv[t] : 0.0f, d1 = h1 ? dinv[r1] : 0.0f;
+    const float *row0 = M + ipls_rowoff(h0 ? t : 0), *row1 = M + ipls_rowoff(h1 ? r1 : 0);
+    for (int j = 0; j < n; ++j) {      // forward: L z = rhs
+        const float dj = dinv[j];
+        const float z0 = __shfl_sync(0xffffffffu, (j < 32) ? a0 : b0, j & 31) * dj;
+        const float z1 = NRHS > 1 ? __shfl_sync(0xffffffffu, (j < 32) ? a1 : b1, j & 31) * dj : 0.0f;
+        if (h0 && t > j) { const float l = row0[j]; a0 -= l * z0; if (NRHS > 1) a1 -= l * z1; }
+        if (h1 && r1 > j) { const float l = row1[j]; b0 -= l * z0; if (NRHS > 1) b1 -= l * z1; }
+    }
+    a0 *= d0; b0 *= d1; a1 *= d0; b1 *= d1;
+    for (int j = n - 1; j >= 0; --j) { // backward: L' x = z
+        const float dj = dinv[j];
+        const float z0 = __shfl_sync(0xffffffffu, (j < 32) ? a0 : b0, j & 31) * dj;
+        const float z1 = NRHS > 1 ? __shfl_sync(0xffffffffu, (j < 32) ? a1 : b1, j & 31) * dj : 0.0f;
+        const float *rowj = M + ipls_rowoff(j);
+        if (t < j) { const float l = rowj[t]; a0 -= l * z0; if (NRHS > 1) a1 -= l * z1; }
+        if (r1 < j) { const float l = rowj[r1]; b0 -= l * z0; if (NRHS > 1) b1 -= l * z1; }
+    }
+    if (h0) { x0[t] = a0 * d0; if (NRHS > 1) x1[t] = a1 * d0; }
+    if (h1) { x0[r1] = b0 * d1; if (NRHS > 1) x1[r1] = b1 * d1; }
+    __syncwarp();
+}
+
+// floats of one team: TEAM == 32 keeps the row-major padded matrix, the CTA team the packed one
+__host__ __device__ inline size_t ipls_generic_vec_floats(int L, int R) { return ((size_t)10 * R + L + 64 + 3) & ~(size_t)3; }
+__host__ __device__ inline size_t ipls_warp_team_floats(int L, int R) {
+    return ipls_generic_vec_floats(L, R) + (size_t)ipls_tri_floats(R);
+}
 __host__ __device__ inline size_t ipls_generic_team_floats(int L, int R) {
     return (size_t)10 * R + L + (size_t)R * (R + 1) / 2 + 64;
 }
@@ -199,9 +282,10 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
     const int teams_per_cta = blockDim.x / TEAM;
     const int team = threadIdx.x / TEAM;
     const int t = Ops::tid();
-    float *base = smem + (size_t)team * ipls_generic_team_floats(L, R);
+    float *base = smem + (size_t)team * (TEAM == 32 ? ipls_warp_team_floats(L, R) : ipls_generic_team_floats(L, R));
     float *a = base, *lam = a + R, *b = lam + R, *w = b + R, *u = w + R, *v = u + R, *da = v + R,
-          *dl = da + R, *dinv = dl + R, *Ga = dinv + R, *yc = Ga + R, *red = yc + L, *Mp = red + 64;
+          *dl = da + R, *dinv = dl + R, *Ga = dinv + R, *yc = Ga + R, *red = yc + L,
+          *Mp = (TEAM == 32) ? base + ipls_generic_vec_floats(L, R) : red + 64;
     const float fR = (float)R;
     const float tau = 0.995f;
 
@@ -313,18 +397,32 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
             ++iters;
             const float mu = gap / fR;
             // ---- Newton matrix M = Gc + diag(lambda / a), packed lower, then Cholesky
-            for (int j = 0; j < R; ++j)
-                for (int i = j + t; i < R; i += TEAM) {
-                    float m = lib.Gc[(size_t)j * R + i];
-                    if (i == j) m += lam[i] / a[i];
-                    Mp[cm(R, i, j)] = m;
-                }
-            Ops::sync();
-            if (team_cholesky<TEAM, float>(Mp, dinv, R, 1e-12f * lib.gdmax)) flags |= LINMIN_INFO_CHOL_REGULARISED;
+            bool regularised;
+            if constexpr (TEAM == 32) {
+                for (int i = 0; i < R; ++i)                  // row i of the lower triangle, row-major
+                    for (int k = t; k <= i; k += 32) {
+                        float m = lib.Gc[(size_t)i * R + k];
+                        if (k == i) m += lam[i] / a[i];
+                        Mp[ipls_rowoff(i) + k] = m;
+                    }
+                Ops::sync();
+                regularised = warp_cholesky_rm(Mp, dinv, R, 1e-12f * lib.gdmax);
+            } else {
+                for (int j = 0; j < R; ++j)
+                    for (int i = j + t; i < R; i += TEAM) {
+                        float m = lib.Gc[(size_t)j * R + i];
+                        if (i == j) m += lam[i] / a[i];
+                        Mp[cm(R, i, j)] = m;
+                    }
+                Ops::sync();
+                regularised = team_cholesky<TEAM, float>(Mp, dinv, R, 1e-12f * lib.gdmax);
+            }
+            if (regularised) flags |= LINMIN_INFO_CHOL_REGULARISED;
             // ---- predictor
             for (int i = t; i < R; i += TEAM) { u[i] = -w[i]; v[i] = 1.0f; }
             Ops::sync();
-            team_solve<TEAM, 2, float>(Mp, dinv, R, u, v);
+            if constexpr (TEAM == 32) warp_solve_rm<2>(Mp, dinv, R, u, v);
+            else team_solve<TEAM, 2, float>(Mp, dinv, R, u, v);
             float su = 0.0f, sv = 0.0f;
             for (int i = t; i < R; i += TEAM) { su += u[i]; sv += v[i]; }
             su = Ops::sum(su, red);
@@ -352,7 +450,8 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
                 u[i] = -w[i] + cc / a[i];
             }
             Ops::sync();
-            team_solve<TEAM, 1, float>(Mp, dinv, R, u, nullptr);
+            if constexpr (TEAM == 32) warp_solve_rm<1>(Mp, dinv, R, u, nullptr);
+            else team_solve<TEAM, 1, float>(Mp, dinv, R, u, nullptr);
             su = 0.0f;
             for (int i = t; i < R; i += TEAM) su += u[i];
             su = Ops::sum(su, red);

@@ -150,7 +150,7 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
         ++launches;
     } else if (R <= 64) {
         const int teams = 8, block = teams * 32;
-        size_t smem = teams * ipls_generic_team_floats(L, R) * sizeof(float);
+        size_t smem = teams * ipls_warp_team_floats(L, R) * sizeof(float);
         CK(cudaFuncSetAttribute(ipls_generic_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int grid = persistent_grid(ipls_generic_kernel<32>, block, smem, lib->sm_count, N, teams);
         ipls_generic_kernel<32><<<grid, block, smem, o.stream>>>(lv, prm);
