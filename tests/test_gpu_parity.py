@@ -266,3 +266,39 @@ def test_results_do_not_depend_on_neighbours_or_repeats(lm, name, N):
         assert np.array_equal(g[key][:m], gs[key], equal_nan=True), f"{key}: shorter batch"
     it, it_p = (g["info"] >> 8) & 0xff, (gp["info"] >> 8) & 0xff
     assert np.array_equal(it[perm], it_p)
+
+
+def test_throughput_full_size_sampled_and_properties(lm):
+    """BASELINE.json configs[4] at its FULL size (128 cubes = 16,777,216 pixels, per-pixel sigma), in the launch
+    configuration bench.py times: 8192 sampled pixels element by element against the oracle, and properties
+    that hold at any size on ALL pixels (simplex feasibility, exact zeros off the support, finite outputs)."""
+    import os
+    import sys
+    import oracle
+    from parity import check_parity
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    from bench import CUBE, gen_cubes
+    n_cubes, L, R = 128, 128, 32
+    N = n_cubes * CUBE
+    Yh = torch.empty((N, L), dtype=torch.float32)
+    Sh = torch.empty((N, L), dtype=torch.float32)
+    A = gen_cubes(0, n_cubes, Yh.numpy(), Sh.numpy(), max(1, (os.cpu_count() or 8)))
+    dev = torch.device("cuda:0")
+    Ad, Yd, Sd = torch.from_numpy(A).to(dev), Yh.to(dev), Sh.to(dev)
+    c, s, r, info, status = lm.unmix(Ad, Yd, Sd)
+    torch.cuda.synchronize()
+    # properties on every pixel (computed on the device by torch: plumbing, not the product)
+    assert bool(torch.isfinite(c).all()) and bool(torch.isfinite(s).all()) and bool(torch.isfinite(r).all())
+    assert float((c.sum(1) - 1.0).abs().max()) <= 1e-5
+    assert float(c.min()) >= 0.0
+    assert bool(((c == 0) == (s == 0)).logical_or(c.gt(0).sum(1, keepdim=True) == 1).all())   # sigma is 0 exactly off the support (and all 0 when k = 1)
+    assert float(r.min()) > 0.0
+    flags = info & 0xff
+    assert int(((flags & 0x10) != 0).sum()) == 0            # no finish fallback
+    assert int(((flags & 0x04) != 0).sum()) == 0            # no non-finite input
+    sel = np.arange(0, N, N // 8192)[:8192]
+    sel_t = torch.from_numpy(sel).to(dev)
+    g = dict(coeffs=c[sel_t].cpu().numpy(), coeff_sigma=s[sel_t].cpu().numpy(), resid=r[sel_t].cpu().numpy())
+    Ys, Ss = Yh.numpy()[sel], Sh.numpy()[sel]
+    ora = oracle.solve(A, Ys, Ss)
+    print(check_parity(A, Ys, Ss, g, ora, label="throughput-full"))
