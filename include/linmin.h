@@ -147,6 +147,11 @@ int linmin_library_last_timing(const linmin_library *lib, float *ipls_ms, float 
  * a few milliseconds of work on `stream` (a cudaStream_t, NULL = default stream).  Not on the hot path. */
 int linmin_probe_fp32_peak(void *stream, double *ffma_tflops, double *ffma2_tflops);
 
+/* Staging memory (per-call workspaces of linmin_unmix_lib, the device buffers of linmin_unmix_host) is taken
+ * from a memory pool the library owns, one per device, and kept between calls.  linmin_trim_memory() returns
+ * what is not in use to the driver (call it when idle; the next call allocates again).  Thread-safe. */
+int linmin_trim_memory(void);
+
 const char *linmin_strerror(int code);
 int linmin_version(void);
 

@@ -32,7 +32,7 @@ INFO_BAD_SIGMA = 0x20
 
 EXPORTS = ["linmin_version", "linmin_strerror", "linmin_library_create", "linmin_library_destroy",
            "linmin_library_last_launches", "linmin_library_enable_timing", "linmin_library_last_timing",
-           "linmin_probe_fp32_peak",
+           "linmin_probe_fp32_peak", "linmin_trim_memory",
            "linmin_unmix_lib", "linmin_unmix", "linmin_unmix_host"]
 
 
@@ -178,6 +178,11 @@ class Library:
             self.destroy()
         except Exception:
             pass
+
+
+def trim_memory() -> None:
+    """Return the library's cached staging memory to the driver."""
+    _check(load().linmin_trim_memory())
 
 
 def probe_fp32_peak(stream=None):
