@@ -602,9 +602,10 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                     double r[NC];
 #pragma unroll
                     for (int c = 0; c < NC; ++c) r[c] = (double)yv[c];
+#pragma unroll 2
                     for (int j = 0; j < kw2; ++j) {
-                        if (resid_due && j < k) {
-                            const double aj = aFs[j];
+                        {   // branch-free: a member beyond this pixel's support subtracts zero
+                            const double aj = (resid_due && j < k) ? aFs[j] : 0.0;
                             const double *row = At64 + (size_t)idx[j] * RS + 2 * t;
 #pragma unroll
                             for (int v = 0; v < LQ; ++v) {
