@@ -212,7 +212,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 }
             }
             int pos = 0;
-#pragma unroll
+#pragma unroll 1
             for (int d = 1; d < 32; ++d) {
                 const int j = (lane + d) & 31;
                 const int kj = __shfl_sync(FULL, kc, j);
@@ -602,7 +602,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                     double r[NC];
 #pragma unroll
                     for (int c = 0; c < NC; ++c) r[c] = (double)yv[c];
-#pragma unroll 2
+#pragma unroll 1
                     for (int j = 0; j < kw2; ++j) {
                         {   // branch-free: a member beyond this pixel's support subtracts zero
                             const double aj = (resid_due && j < k) ? aFs[j] : 0.0;
@@ -626,7 +626,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 }
                 // ---- g_i = A_i'r for every endmember (FFMA2 over my channels), partial sums exchanged
                 //      through Ex[lane][chunk ^ lane]; lane t ends with endmembers 4 t .. 4 t + 3
-#pragma unroll 4
+#pragma unroll 1
                 for (int c4 = 0; c4 < RP / 4; ++c4) {
                     float pr[4];
 #pragma unroll
@@ -730,7 +730,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                     for (int c = 0; c < NC / 2; ++c) d[ii][c] = make_float2(0.0f, 0.0f);
                 // branch-free body (a pixel whose support ends before j, or that has no J to form, multiplies
                 // by zero): the loads of step j + 1 can be issued under the FFMA2 stream of step j
-#pragma unroll 2
+#pragma unroll 1
                 for (int j = 0; j < kj; ++j) {
                     const bool on = doj && j < k && ib < k;
                     float hh[IT];
