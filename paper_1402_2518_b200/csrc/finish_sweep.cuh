@@ -363,6 +363,10 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             const bool need0 = act && t < k && !((have >> i0) & 1u);
             const bool need1 = act && t + 8 < k && !((have >> i1) & 1u);
             if (__any_sync(FULL, need0 || need1)) {
+                double yd[NC];                      // widened once per round, not once per member
+#pragma unroll
+                for (int c = 0; c < NC; ++c) yd[c] = (double)yv[c];
+#pragma unroll 1
                 for (int j = 0; j < kw; ++j) {
                     const int ij = idx[j];
                     if (act && j < k && !((have >> ij) & 1u)) {
@@ -372,8 +376,8 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                         for (int v = 0; v < LQ; ++v) {
                             const double2 lo = *reinterpret_cast<const double2 *>(row + 16 * v);
                             const double2 hi = *reinterpret_cast<const double2 *>(row + RS / 2 + 16 * v);
-                            s0 = fma(lo.x, (double)yv[4 * v + 0], s0); s1 = fma(lo.y, (double)yv[4 * v + 1], s1);
-                            s2 = fma(hi.x, (double)yv[4 * v + 2], s2); s3 = fma(hi.y, (double)yv[4 * v + 3], s3);
+                            s0 = fma(lo.x, yd[4 * v + 0], s0); s1 = fma(lo.y, yd[4 * v + 1], s1);
+                            s2 = fma(hi.x, yd[4 * v + 2], s2); s3 = fma(hi.y, yd[4 * v + 3], s3);
                         }
                         Md[j * 8 + t] = (s0 + s1) + (s2 + s3);
                     }
@@ -397,9 +401,9 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             if (act) {
                 bR[t] = (t < k) ? bE[i0] : 0.0;
                 if (wide) bR[t + 8] = (t + 8 < k) ? bE[i1] : 0.0;
-#pragma unroll
-                for (int c2 = 0; c2 < 8; ++c2) {
-                    if (c2 < 4 || wide) {
+#pragma unroll 1
+                for (int c2 = 0; c2 < (wide ? 8 : 4); ++c2) {
+                    {
                         const int2 jj = *reinterpret_cast<const int2 *>(idx + 2 * c2);
                         const bool v0 = 2 * c2 < k, v1 = 2 * c2 + 1 < k;
                         double2 m0, m1;
@@ -420,10 +424,6 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             for (int j = 0; j < kw; ++j) {
                 const bool on = act && rej < 0 && j < k;
                 const double *Mj = Md + j * MS;
-                double2 rj[8];
-#pragma unroll
-                for (int c2 = 0; c2 < 8; ++c2)
-                    if (c2 < 4 || wide) rj[c2] = *reinterpret_cast<const double2 *>(Mj + 2 * c2);
                 const double d = Mj[j];
                 const int ij = idx[j];
                 const bool ok = d > 1e-13 * G64s[ij * GS + ij];
@@ -433,26 +433,29 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 double f0 = M0[j] * pv, f1 = 0.0;
                 if (t == j) f0 = 1.0 - pv;                      // pivot row: m - (1 - p) m = p m
                 if (wide) { f1 = M1[j] * pv; if (t + 8 == j) f1 = 1.0 - pv; }
-                __syncwarp();                                   // row j was read by everybody
-                if (go && t < k) {
-#pragma unroll
-                    for (int c2 = 0; c2 < 8; ++c2) {
-                        if (c2 < 4 || wide) {
+                // row j goes to a line of its own (qv is free until the point is accepted): the update loops can
+                // then stay rolled -- this kernel is bound by instruction supply, not by arithmetic
+                *reinterpret_cast<double2 *>(qv + 2 * t) = *reinterpret_cast<const double2 *>(Mj + 2 * t);
+                __syncwarp();
+                if (go) {
+                    const int nc2 = wide ? 8 : 4;
+                    const bool r0 = t < k, r1 = wide && t + 8 < k;
+#pragma unroll 1
+                    for (int c2 = 0; c2 < nc2; ++c2) {
+                        const double2 r = *reinterpret_cast<const double2 *>(qv + 2 * c2);
+                        if (r0) {
                             double2 m = *reinterpret_cast<double2 *>(M0 + 2 * c2);
-                            m.x = fma(-f0, rj[c2].x, m.x); m.y = fma(-f0, rj[c2].y, m.y);
+                            m.x = fma(-f0, r.x, m.x); m.y = fma(-f0, r.y, m.y);
                             *reinterpret_cast<double2 *>(M0 + 2 * c2) = m;
                         }
+                        if (r1) {
+                            double2 m = *reinterpret_cast<double2 *>(M1 + 2 * c2);
+                            m.x = fma(-f1, r.x, m.x); m.y = fma(-f1, r.y, m.y);
+                            *reinterpret_cast<double2 *>(M1 + 2 * c2) = m;
+                        }
                     }
-                    M0[j] = (t == j) ? pv : -f0;
-                }
-                if (wide && go && t + 8 < k) {
-#pragma unroll
-                    for (int c2 = 0; c2 < 8; ++c2) {
-                        double2 m = *reinterpret_cast<double2 *>(M1 + 2 * c2);
-                        m.x = fma(-f1, rj[c2].x, m.x); m.y = fma(-f1, rj[c2].y, m.y);
-                        *reinterpret_cast<double2 *>(M1 + 2 * c2) = m;
-                    }
-                    M1[j] = (t + 8 == j) ? pv : -f1;
+                    if (r0) M0[j] = (t == j) ? pv : -f0;
+                    if (r1) M1[j] = (t + 8 == j) ? pv : -f1;
                 }
                 __syncwarp();
             }
@@ -494,9 +497,9 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             q0 = 0.0; q1 = 0.0;
             double x0 = 0.0, x1 = 0.0;
             if (!skip) {
-#pragma unroll
-                for (int c2 = 0; c2 < 8; ++c2) {
-                    if (c2 < 4 || wide) {
+#pragma unroll 1
+                for (int c2 = 0; c2 < (wide ? 8 : 4); ++c2) {
+                    {
                         const double2 bb = *reinterpret_cast<const double2 *>(bR + 2 * c2);
                         const double2 m = *reinterpret_cast<const double2 *>(M0 + 2 * c2);
                         q0 += m.x + m.y;
