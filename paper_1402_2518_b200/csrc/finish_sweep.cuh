@@ -460,25 +460,25 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 __syncwarp();
             }
             bool skip = !act;
-            if (act && rej >= 0) {
-                // A_F lost rank at member `rej` (R9): drop it, block it, stay at the same point
-                skip = true;
-                if (t == (rej & 7)) state[(rej < 8) ? i0 : i1] = 2;
-                const int n0 = t - (t > rej ? 1 : 0), n1 = t + 8 - (t + 8 > rej ? 1 : 0);
-                const bool k0 = (t < k) && (t != rej), k1 = (t + 8 < k) && (t + 8 != rej);
-                if (k0) { idx[n0] = i0; aFs[n0] = a0; }
-                if (k1) { idx[n1] = i1; aFs[n1] = a1; }
-                --k; last_added = -1;
-                ++pivots;
-            }
-            __syncwarp();
-            if (act && rej >= 0) {
-                a0 = 0.0; a1 = 0.0; i0 = 0; i1 = 0;
-                if (t < k) { a0 = aFs[t]; i0 = idx[t]; }
-                if (t + 8 < k) { a1 = aFs[t + 8]; i1 = idx[t + 8]; }
-            }
             bool fell = false;      // this round ended in the fallback state: the residual is still due
-            {
+            if (__any_sync(FULL, act && rej >= 0)) {       // warp-uniform and rare (duplicate or collinear members)
+                if (act && rej >= 0) {
+                    // A_F lost rank at member `rej` (R9): drop it, block it, stay at the same point
+                    skip = true;
+                    if (t == (rej & 7)) state[(rej < 8) ? i0 : i1] = 2;
+                    const int n0 = t - (t > rej ? 1 : 0), n1 = t + 8 - (t + 8 > rej ? 1 : 0);
+                    const bool k0 = (t < k) && (t != rej), k1 = (t + 8 < k) && (t + 8 != rej);
+                    if (k0) { idx[n0] = i0; aFs[n0] = a0; }
+                    if (k1) { idx[n1] = i1; aFs[n1] = a1; }
+                    --k; last_added = -1;
+                    ++pivots;
+                }
+                __syncwarp();
+                if (act && rej >= 0) {
+                    a0 = 0.0; a1 = 0.0; i0 = 0; i1 = 0;
+                    if (t < k) { a0 = aFs[t]; i0 = idx[t]; }
+                    if (t + 8 < k) { a1 = aFs[t + 8]; i1 = idx[t + 8]; }
+                }
                 const double s = gsum(a0 + a1);
                 if (act && rej >= 0) {
                     if (k == 0 || pivots > max_pivots) {
@@ -490,8 +490,8 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                         if (t + 8 < k) aFs[t + 8] = a1;
                     }
                 }
+                __syncwarp();
             }
-            __syncwarp();
 
             // ---- q = K 1 and x = K b_F from my rows; trial point x - mu q with 1'(x - mu q) = 1
             q0 = 0.0; q1 = 0.0;
@@ -523,33 +523,43 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 const bool m0 = t < k, m1 = t + 8 < k;
                 const double amin = gmin(fmin(m0 ? t0v : INFINITY, m1 ? t1v : INFINITY));
                 const bool ratio = !skip && !(amin > 0.0);
-                // ---- ratio step towards the trial point until the first coefficient reaches zero; drop it
-                double r0 = INFINITY, r1 = INFINITY;
-                if (m0 && !(t0v > 0.0)) { const double den = a0 - t0v; r0 = den > 0.0 ? a0 * rcp_d(fmax(den, 1e-30)) : 0.0; }
-                if (m1 && !(t1v > 0.0)) { const double den = a1 - t1v; r1 = den > 0.0 ? a1 * rcp_d(fmax(den, 1e-30)) : 0.0; }
-                double alpha = fmin(1.0, gmin(fmin(r0, r1)));
-                if (alpha < 0.0) alpha = 0.0;
-                const double n0v = a0 + alpha * (t0v - a0), n1v = a1 + alpha * (t1v - a1);
-                const bool b0 = r0 <= alpha, b1 = r1 <= alpha;
-                const bool keep0 = m0 && !b0 && (n0v > 0.0), keep1 = m1 && !b1 && (n1v > 0.0);
-                // ranks of the kept members: ballots over the group, slot 0 members come first
-                const unsigned bk0 = (__ballot_sync(FULL, keep0) >> (8 * g)) & 0xffu;
-                const unsigned bk1 = (__ballot_sync(FULL, keep1) >> (8 * g)) & 0xffu;
-                const double ssum = gsum((keep0 ? n0v : 0.0) + (keep1 ? n1v : 0.0));
-                __syncwarp();       // every read of idx / aFs of this round precedes the writes below
-                if (ratio) {
-                    if (m0 && !keep0) state[i0] = (i0 == last_added && alpha == 0.0) ? 2 : 0;
-                    if (m1 && !keep1) state[i1] = (i1 == last_added && alpha == 0.0) ? 2 : 0;
-                    const int k0r = __popc(bk0 & ((1u << t) - 1u));
-                    const int k1r = __popc(bk0) + __popc(bk1 & ((1u << t) - 1u));
-                    const double rs = rcp_d(ssum > 0.0 ? ssum : 1.0);
-                    if (keep0) { idx[k0r] = i0; aFs[k0r] = n0v * rs; }
-                    if (keep1) { idx[k1r] = i1; aFs[k1r] = n1v * rs; }
-                    k = __popc(bk0) + __popc(bk1);
-                    last_added = -1;
-                    ++pivots;
-                    if (k == 0 || pivots > max_pivots) { st = 2; fell = true; }
-                } else if (!skip) {
+                // ---- ratio step towards the trial point until the first coefficient reaches zero; drop it.
+                //      Warp-uniform branch: 86 % of the rounds accept the trial point and skip all of this.
+                if (__any_sync(FULL, ratio)) {
+                    double r0 = INFINITY, r1 = INFINITY;
+                    if (m0 && !(t0v > 0.0)) { const double den = a0 - t0v; r0 = den > 0.0 ? a0 * rcp_d(fmax(den, 1e-30)) : 0.0; }
+                    if (m1 && !(t1v > 0.0)) { const double den = a1 - t1v; r1 = den > 0.0 ? a1 * rcp_d(fmax(den, 1e-30)) : 0.0; }
+                    double alpha = fmin(1.0, gmin(fmin(r0, r1)));
+                    if (alpha < 0.0) alpha = 0.0;
+                    const double n0v = a0 + alpha * (t0v - a0), n1v = a1 + alpha * (t1v - a1);
+                    const bool b0 = r0 <= alpha, b1 = r1 <= alpha;
+                    const bool keep0 = m0 && !b0 && (n0v > 0.0), keep1 = m1 && !b1 && (n1v > 0.0);
+                    // ranks of the kept members: ballots over the group, slot 0 members come first
+                    const unsigned bk0 = (__ballot_sync(FULL, keep0) >> (8 * g)) & 0xffu;
+                    const unsigned bk1 = (__ballot_sync(FULL, keep1) >> (8 * g)) & 0xffu;
+                    const double ssum = gsum((keep0 ? n0v : 0.0) + (keep1 ? n1v : 0.0));
+                    __syncwarp();       // every read of idx / aFs of this round precedes the writes below
+                    if (ratio) {
+                        if (m0 && !keep0) state[i0] = (i0 == last_added && alpha == 0.0) ? 2 : 0;
+                        if (m1 && !keep1) state[i1] = (i1 == last_added && alpha == 0.0) ? 2 : 0;
+                        const int k0r = __popc(bk0 & ((1u << t) - 1u));
+                        const int k1r = __popc(bk0) + __popc(bk1 & ((1u << t) - 1u));
+                        const double rs = rcp_d(ssum > 0.0 ? ssum : 1.0);
+                        if (keep0) { idx[k0r] = i0; aFs[k0r] = n0v * rs; }
+                        if (keep1) { idx[k1r] = i1; aFs[k1r] = n1v * rs; }
+                        k = __popc(bk0) + __popc(bk1);
+                        last_added = -1;
+                        ++pivots;
+                        if (k == 0 || pivots > max_pivots) { st = 2; fell = true; }
+                    }
+                    __syncwarp();
+                    if (ratio) {
+                        a0 = 0.0; a1 = 0.0; i0 = 0; i1 = 0;
+                        if (t < k) { a0 = aFs[t]; i0 = idx[t]; }
+                        if (t + 8 < k) { a1 = aFs[t + 8]; i1 = idx[t + 8]; }
+                    }
+                }
+                if (!ratio && !skip) {
                     accepted = true;
                     a0 = m0 ? t0v : 0.0; a1 = m1 ? t1v : 0.0;
                     if (m0) aFs[t] = a0;
@@ -559,11 +569,6 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                     qv[t + 8] = q1;
                 }
                 __syncwarp();
-                if (ratio) {
-                    a0 = 0.0; a1 = 0.0; i0 = 0; i1 = 0;
-                    if (t < k) { a0 = aFs[t]; i0 = idx[t]; }
-                    if (t + 8 < k) { a1 = aFs[t + 8]; i1 = idx[t + 8]; }
-                }
             }
             // ---- H = K - q q'/(1'q) (fp32) replaces the swept matrix: read my rows, then write them
             const bool resid_due = accepted || fell;
