@@ -440,7 +440,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 if (go) {
                     const int nc2 = wide ? 8 : 4;
                     const bool r0 = t < k, r1 = wide && t + 8 < k;
-#pragma unroll 1
+#pragma unroll 4
                     for (int c2 = 0; c2 < nc2; ++c2) {
                         const double2 r = *reinterpret_cast<const double2 *>(qv + 2 * c2);
                         if (r0) {
