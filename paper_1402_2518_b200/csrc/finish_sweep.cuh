@@ -42,7 +42,7 @@ constexpr int PIX_BYTES = OFF_STATE + 32;     // 3232
 static_assert(PIX_BYTES % 16 == 0, "scratch alignment");
 
 __host__ __device__ inline size_t cta_bytes(int LQ) {
-    return (size_t)RP * GS * 8 + (size_t)RP * 32 * LQ * 8 + (size_t)RP * 32 * LQ * 4;
+    return (size_t)RP * GS * 8 + (size_t)RP * 32 * LQ * 4;
 }
 
 __device__ __forceinline__ double gsum(double v) {
@@ -146,8 +146,8 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int L = lib.L, R = lib.R;
     double *G64s = (double *)smem_raw;                                    // [RP][GS]
-    double *At64 = (double *)(smem_raw + (size_t)RP * GS * 8);            // [RP][2][8 LQ][2]
-    float *At32 = (float *)(At64 + (size_t)RP * RS);                      // [RP][32 LQ]
+    float *At32 = (float *)(smem_raw + (size_t)RP * GS * 8);              // [RP][32 LQ]: library rows, fp32 (widened on the fly:
+                                                                          // an fp64 copy costs twice the shared-memory wavefronts)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 3, t = lane & 7;
     unsigned char *S = (unsigned char *)(At32 + (size_t)RP * RS) + (size_t)(warp * 4 + g) * PIX_BYTES;
     double *Md = (double *)(S + OFF_M);
@@ -162,7 +162,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
     int *idx = (int *)(S + OFF_IDX);
     unsigned char *state = S + OFF_STATE;
 
-    // ---- once per CTA: stage the library (transposed; fp64 copy split in two planes per float4)
+    // ---- once per CTA: stage the library (transposed, fp32) and the fp64 Gram matrix
     for (int e = threadIdx.x; e < RP * RP; e += blockDim.x) {
         const int i = e >> 5, j = e & 31;
         G64s[i * GS + j] = (i < R && j < R) ? lib.G64[i * R + j] : 0.0;
@@ -171,8 +171,6 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
         const int r = e / RS, l = e - r * RS;
         const float a = (r < R && l < L) ? lib.A[(size_t)l * R + r] : 0.0f;
         At32[e] = a;
-        const int c = l >> 2, q = l & 3;
-        At64[(size_t)r * RS + (q >> 1) * (RS / 2) + c * 2 + (q & 1)] = (double)a;
     }
     __syncthreads();
 
@@ -370,14 +368,13 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 for (int j = 0; j < kw; ++j) {
                     const int ij = idx[j];
                     if (act && j < k && !((have >> ij) & 1u)) {
-                        const double *row = At64 + (size_t)ij * RS + 2 * t;
+                        const float *row = At32 + (size_t)ij * RS + 4 * t;
                         double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
 #pragma unroll
                         for (int v = 0; v < LQ; ++v) {
-                            const double2 lo = *reinterpret_cast<const double2 *>(row + 16 * v);
-                            const double2 hi = *reinterpret_cast<const double2 *>(row + RS / 2 + 16 * v);
-                            s0 = fma(lo.x, yd[4 * v + 0], s0); s1 = fma(lo.y, yd[4 * v + 1], s1);
-                            s2 = fma(hi.x, yd[4 * v + 2], s2); s3 = fma(hi.y, yd[4 * v + 3], s3);
+                            const float4 a4 = *reinterpret_cast<const float4 *>(row + 32 * v);
+                            s0 = fma((double)a4.x, yd[4 * v + 0], s0); s1 = fma((double)a4.y, yd[4 * v + 1], s1);
+                            s2 = fma((double)a4.z, yd[4 * v + 2], s2); s3 = fma((double)a4.w, yd[4 * v + 3], s3);
                         }
                         Md[j * 8 + t] = (s0 + s1) + (s2 + s3);
                     }
@@ -614,13 +611,12 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                     for (int j = 0; j < kw2; ++j) {
                         {   // branch-free: a member beyond this pixel's support subtracts zero
                             const double aj = (resid_due && j < k) ? aFs[j] : 0.0;
-                            const double *row = At64 + (size_t)idx[j] * RS + 2 * t;
+                            const float *row = At32 + (size_t)idx[j] * RS + 4 * t;
 #pragma unroll
                             for (int v = 0; v < LQ; ++v) {
-                                const double2 lo = *reinterpret_cast<const double2 *>(row + 16 * v);
-                                const double2 hi = *reinterpret_cast<const double2 *>(row + RS / 2 + 16 * v);
-                                r[4 * v + 0] = fma(-lo.x, aj, r[4 * v + 0]); r[4 * v + 1] = fma(-lo.y, aj, r[4 * v + 1]);
-                                r[4 * v + 2] = fma(-hi.x, aj, r[4 * v + 2]); r[4 * v + 3] = fma(-hi.y, aj, r[4 * v + 3]);
+                                const float4 a4 = *reinterpret_cast<const float4 *>(row + 32 * v);
+                                r[4 * v + 0] = fma(-(double)a4.x, aj, r[4 * v + 0]); r[4 * v + 1] = fma(-(double)a4.y, aj, r[4 * v + 1]);
+                                r[4 * v + 2] = fma(-(double)a4.z, aj, r[4 * v + 2]); r[4 * v + 3] = fma(-(double)a4.w, aj, r[4 * v + 3]);
                             }
                         }
                     }
