@@ -15,6 +15,7 @@ namespace linmin {
 struct LibView {
     int L, R;
     const float *A;     // L x R, caller's library (copied into the handle)
+    const float *At;    // R x L, the same by endmember (At[r][l] = A[l][r])
     const float *Ac;    // L x R, centred: Ac[l][r] = A[l][r] - c[l], c[l] = mean_r A[l][r]
     const float *c;     // L
     const float *Gc;    // R x R fp32, Gc = Ac' Ac accumulated in fp64 (drives IPLS)

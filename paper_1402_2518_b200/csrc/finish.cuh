@@ -49,7 +49,8 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
     float *r32 = y + L, *Hs = r32 + L, *g = Hs + (size_t)KMAX * (KMAX + 1) / 2;
     int *idx = (int *)(g + R);
     unsigned char *state = (unsigned char *)(idx + KMAX);
-    const float *A = lib.A;
+    const float *A = lib.A;      // by channel: the multiplier pass walks the endmembers across the lanes
+    const float *At = lib.At;    // by endmember: every pass over the channels of one member reads consecutive addresses
     const int max_pivots = 4 * KMAX + 8;
 
     for (int64_t p = (int64_t)blockIdx.x * warps + warp; p < prm.N; p += (int64_t)gridDim.x * warps) {
@@ -165,14 +166,14 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
             // ---- data-space residual at the current point and its projection on the support
             for (int l = lane; l < L; l += 32) {
                 double s = (double)y[l];
-                for (int j = 0; j < k; ++j) s -= (double)A[(size_t)l * R + idx[j]] * aF[j];
+                for (int j = 0; j < k; ++j) s -= (double)At[(size_t)idx[j] * L + l] * aF[j];
                 r[l] = s;
             }
             __syncwarp();
             double suma = 0.0;
             for (int j = 0; j < k; ++j) {
                 double s = 0.0;
-                for (int l = lane; l < L; l += 32) s += (double)A[(size_t)l * R + idx[j]] * r[l];
+                for (int l = lane; l < L; l += 32) s += (double)At[(size_t)idx[j] * L + l] * r[l];
                 s = warp_sum(s);
                 if (lane == 0) { gF[j] = s; atry[j] = s; }
                 suma += aF[j];
@@ -233,7 +234,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
             __syncwarp();
             for (int l = lane; l < L; l += 32) {
                 double s = (double)y[l];
-                for (int j = 0; j < k; ++j) s -= (double)A[(size_t)l * R + idx[j]] * aF[j];
+                for (int j = 0; j < k; ++j) s -= (double)At[(size_t)idx[j] * L + l] * aF[j];
                 r[l] = s;
                 r32[l] = (float)s;
             }
@@ -241,7 +242,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
             nu = 0.0;
             for (int j = 0; j < k; ++j) {
                 double s = 0.0;
-                for (int l = lane; l < L; l += 32) s += (double)A[(size_t)l * R + idx[j]] * r[l];
+                for (int l = lane; l < L; l += 32) s += (double)At[(size_t)idx[j] * L + l] * r[l];
                 s = warp_sum(s);
                 nu += s * aF[j];
             }
@@ -276,7 +277,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
             // residual at the current feasible point
             for (int l = lane; l < L; l += 32) {
                 double s = (double)y[l];
-                for (int j = 0; j < k; ++j) s -= (double)A[(size_t)l * R + idx[j]] * aF[j];
+                for (int j = 0; j < k; ++j) s -= (double)At[(size_t)idx[j] * L + l] * aF[j];
                 r[l] = s;
             }
             __syncwarp();
@@ -339,7 +340,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
                         float d = 0.0f;
                         for (int j = 0; j < k; ++j) {
                             float h = (i >= j) ? Hs[cm(k, i, j)] : Hs[cm(k, j, i)];
-                            d = fmaf(h, A[(size_t)l * R + idx[j]], d);
+                            d = fmaf(h, At[(size_t)idx[j] * L + l], d);
                         }
                         float sv = sg ? sg[l] : 1.0f;
                         d *= sv;

@@ -33,7 +33,7 @@ struct linmin_library {
     int device = 0;
     int sm_count = 0;
     cudaStream_t stream = nullptr;   // stream the handle was created on (frees are ordered on it)
-    float *A = nullptr, *Ac = nullptr, *c = nullptr, *Gc = nullptr, *Gi = nullptr, *Giq = nullptr;
+    float *A = nullptr, *At = nullptr, *Ac = nullptr, *c = nullptr, *Gc = nullptr, *Gi = nullptr, *Giq = nullptr;
     double *G64 = nullptr;
     float gdmax = 0.0f;
     mutable int last_launches = 0;
@@ -140,7 +140,7 @@ int check_sizes(int64_t N, int L, int R) {
 
 LibView view_of(const linmin_library *lib) {
     LibView v;
-    v.L = lib->L; v.R = lib->R; v.A = lib->A; v.Ac = lib->Ac; v.c = lib->c; v.Gc = lib->Gc;
+    v.L = lib->L; v.R = lib->R; v.A = lib->A; v.At = lib->At; v.Ac = lib->Ac; v.c = lib->c; v.Gc = lib->Gc;
     v.G64 = lib->G64; v.gdmax = lib->gdmax; v.Gi = lib->Gi; v.Giq = lib->Giq;
     return v;
 }
@@ -253,6 +253,7 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
     CKF(cudaDeviceGetAttribute(&lib->sm_count, cudaDevAttrMultiProcessorCount, dev));
     const size_t LR = (size_t)L * R, RR = (size_t)R * R;
     CKF(cudaMallocAsync((void **)&lib->A, LR * sizeof(float), stream));
+    CKF(cudaMallocAsync((void **)&lib->At, LR * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->Ac, LR * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->c, (size_t)L * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->Gc, RR * sizeof(float), stream));
@@ -263,6 +264,8 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
     {
         int block = 256, grid = (L * 32 + block - 1) / block;
         center_library_kernel<<<grid, block, 0, stream>>>(lib->A, L, R, lib->Ac, lib->c, flags);
+        CKF(cudaGetLastError());
+        transpose_library_kernel<<<(int)((LR + block - 1) / block), block, 0, stream>>>(lib->A, L, R, lib->At);
         CKF(cudaGetLastError());
         grid = (int)((RR + block - 1) / block);
         gram_kernel<<<grid, block, 0, stream>>>(lib->A, lib->Ac, L, R, lib->G64, lib->Gc);
@@ -388,6 +391,7 @@ void linmin_library_destroy(linmin_library *lib) {
     if (!lib) return;
     cudaStream_t s = lib->stream;
     if (lib->A) cudaFreeAsync(lib->A, s);
+    if (lib->At) cudaFreeAsync(lib->At, s);
     if (lib->Ac) cudaFreeAsync(lib->Ac, s);
     if (lib->c) cudaFreeAsync(lib->c, s);
     if (lib->Gc) cudaFreeAsync(lib->Gc, s);

@@ -10,6 +10,15 @@
 
 namespace linmin {
 
+// At[r][l] = A[l][r]: the library by endmember, for the kernels that walk one endmember over the channels
+// (the lanes of a warp then read consecutive addresses).  One thread per element, reads coalesced.
+__global__ void transpose_library_kernel(const float *__restrict__ A, int L, int R, float *__restrict__ At) {
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= (size_t)L * R) return;
+    const int l = (int)(e / R), r = (int)(e - (size_t)l * R);
+    At[(size_t)r * L + l] = A[e];
+}
+
 // one warp per channel l: c[l] = mean_r A[l][r] (fp64), Ac[l][r] = fl32(A[l][r] - c[l]).
 // flags[0] |= 1 when A holds a non-finite value.
 __global__ void center_library_kernel(const float *__restrict__ A, int L, int R, float *__restrict__ Ac,
