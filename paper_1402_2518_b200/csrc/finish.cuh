@@ -249,8 +249,16 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
             // multipliers lambda_i = nu - A_i'r off the support (fp32 dot products of the fp64 residual)
             float lmin = INFINITY; int jmin = -1; float gmax = 0.0f;
             for (int i = lane; i < R; i += 32) {
-                float s = 0.0f;
-                for (int l = 0; l < L; ++l) s = fmaf(A[(size_t)l * R + i], r32[l], s);
+                float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f, s3 = 0.0f;      // four chains: the loads of a chain overlap
+                int l = 0;
+                for (; l + 3 < L; l += 4) {
+                    s0 = fmaf(A[(size_t)(l + 0) * R + i], r32[l + 0], s0);
+                    s1 = fmaf(A[(size_t)(l + 1) * R + i], r32[l + 1], s1);
+                    s2 = fmaf(A[(size_t)(l + 2) * R + i], r32[l + 2], s2);
+                    s3 = fmaf(A[(size_t)(l + 3) * R + i], r32[l + 3], s3);
+                }
+                for (; l < L; ++l) s0 = fmaf(A[(size_t)l * R + i], r32[l], s0);
+                const float s = (s0 + s1) + (s2 + s3);
                 gmax = fmaxf(gmax, fabsf(s));
                 if (state[i] == 0) {
                     float li = (float)nu - s;
@@ -334,21 +342,53 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
                     }
                 __syncwarp();
                 const float *sg = prm.has_sigma ? prm.sigma + p * prm.sigma_stride : nullptr;
-                for (int i = 0; i < k; ++i) {
-                    float acc = 0.0f;
-                    for (int l = lane; l < L; l += 32) {
-                        float d = 0.0f;
-                        for (int j = 0; j < k; ++j) {
-                            float h = (i >= j) ? Hs[cm(k, i, j)] : Hs[cm(k, j, i)];
-                            d = fmaf(h, At[(size_t)idx[j] * L + l], d);
-                        }
-                        float sv = sg ? sg[l] : 1.0f;
-                        d *= sv;
-                        acc = fmaf(d, d, acc);
+                // J = H A_F' as a small matrix product per chunk of 256 channels (8 per lane): four rows of H at a
+                // time, so that a member's library values are loaded once per four rows and H once per 8 channels
+                for (int i = lane; i < k; i += 32) tmp[i] = 0.0;
+                __syncwarp();
+                for (int l0 = 0; l0 < L; l0 += 256) {
+                    float sv[8];
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const int l = l0 + lane + 32 * c;
+                        sv[c] = (l < L) ? (sg ? sg[l] : 1.0f) : 0.0f;
                     }
-                    acc = warp_sum(acc);
-                    if (lane == 0) sout[idx[i]] = sqrtf(acc);
+                    for (int i0 = 0; i0 < k; i0 += 4) {
+                        float d[4][8];
+#pragma unroll
+                        for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) d[ii][c] = 0.0f;
+                        for (int j = 0; j < k; ++j) {
+                            const float *row = At + (size_t)idx[j] * L + l0 + lane;
+                            float a[8], h[4];
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) a[c] = (l0 + lane + 32 * c < L) ? row[32 * c] : 0.0f;
+#pragma unroll
+                            for (int ii = 0; ii < 4; ++ii) {
+                                const int i = i0 + ii;
+                                h[ii] = (i < k) ? ((i >= j) ? Hs[cm(k, i, j)] : Hs[cm(k, j, i)]) : 0.0f;
+                            }
+#pragma unroll
+                            for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+                                for (int c = 0; c < 8; ++c) d[ii][c] = fmaf(h[ii], a[c], d[ii][c]);
+                        }
+#pragma unroll
+                        for (int ii = 0; ii < 4; ++ii) {
+                            float acc = 0.0f;
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) {
+                                const float dv = d[ii][c] * sv[c];
+                                acc = fmaf(dv, dv, acc);
+                            }
+                            acc = warp_sum(acc);
+                            if (lane == 0 && i0 + ii < k) tmp[i0 + ii] += (double)acc;
+                        }
+                    }
                 }
+                __syncwarp();
+                for (int i = lane; i < k; i += 32) sout[idx[i]] = sqrtf((float)tmp[i]);
             }
         }
         if (prm.info && lane == 0) {
