@@ -119,6 +119,15 @@ class ClockSampler:
                 "power_w_max": float(max(power)), "reasons": sorted(reasons)}
 
 
+def host_threads():
+    """Threads for the oracle legs: the host cores this process may use.  Passed explicitly, because torchrun
+    presets OMP_NUM_THREADS=1 for its workers and the oracle would otherwise run on one core there."""
+    try:
+        return max(1, len(os.sched_getaffinity(0)))
+    except AttributeError:
+        return max(1, os.cpu_count() or 1)
+
+
 def run_reference(args, rank, world):
     """--impl reference: the CPU oracle as it stands, on a bounded sample of the same workload."""
     if rank != 0:
@@ -132,12 +141,12 @@ def run_reference(args, rank, world):
     Y, s, _, _ = make_cube(cfg, A64, rng, CUBE)
     Y, s = Y[:n], s[:n]
     A = A64.astype(np.float32)
-    cores = oracle.max_threads()
+    cores = host_threads()
     for _ in range(args.warmup):
-        oracle.solve(A, Y[: max(1, n // 8)], s[: max(1, n // 8)])
+        oracle.solve(A, Y[: max(1, n // 8)], s[: max(1, n // 8)], nthreads=cores)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle.solve(A, Y, s)
+        oracle.solve(A, Y, s, nthreads=cores)
     dt = (time.perf_counter() - t0) / args.steps
     v = n / dt
     sample = f"first {n} pixels of cube 0 of config 4 per step"
@@ -300,9 +309,9 @@ def main():
         if not args.no_cpu_baseline:
             n = 262144 if args.sample is None else args.sample
             n = min(n, N)
-            cores = oracle.max_threads()
+            cores = host_threads()
             t0 = time.perf_counter()
-            oracle.solve(A, Yh.numpy()[:n], Sh.numpy()[:n])
+            oracle.solve(A, Yh.numpy()[:n], Sh.numpy()[:n], nthreads=cores)
             dt = time.perf_counter() - t0
             cpu_baseline = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                             "sample": f"first {n} pixels of the same workload, one pass, {dt:.1f} s"}
