@@ -8,6 +8,11 @@
 
 // an endmember belongs to the initial support of the finish when its IPLS coefficient exceeds this
 #define LINMIN_SUPPORT_THRESHOLD 1e-4f
+// ... and IPLS hands over a_i = 0 where the primal-dual indicator says "inactive": a_i sc <= kappa lambda_i
+// (sc = the pixel's gradient scale).  At the stopping point a_i lambda_i ~ mu for every i, so a_i / lambda_i
+// separates the two classes by orders of magnitude where a_i alone does not; kappa = 30 halves the support
+// repairs of the finish against the plain threshold (numpy model of the iteration on config 4).
+#define LINMIN_TAPIA_KAPPA 30.0f
 
 namespace linmin {
 

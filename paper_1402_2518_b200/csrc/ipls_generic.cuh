@@ -478,7 +478,8 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
             nu = fmaf(ad, dnu, nu);
             Ops::sync();
         }
-        for (int i = t; i < R; i += TEAM) prm.coeffs[p * R + i] = a[i];
+        // hand-over: zero where the primal-dual indicator says inactive (LINMIN_TAPIA_KAPPA, common.cuh)
+        for (int i = t; i < R; i += TEAM) prm.coeffs[p * R + i] = (a[i] * sc > LINMIN_TAPIA_KAPPA * lam[i]) ? a[i] : 0.0f;
         if (prm.info && t == 0) prm.info[p] = flags | (iters << 8);
         Ops::sync();
     }

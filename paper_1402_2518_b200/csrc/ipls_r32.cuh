@@ -651,7 +651,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         // ---- store the iterate (coalesced: 8 lanes x float4 = one 128 B row) and the info word
         __syncwarp();
 #pragma unroll
-        for (int s = 0; s < 4; ++s) xb0[t + 8 * s] = a[s];
+        for (int s = 0; s < 4; ++s) xb0[t + 8 * s] = (a[s] * sc > LINMIN_TAPIA_KAPPA * lam[s]) ? a[s] : 0.0f;
         __syncwarp();
         if (valid) {
             float4 o = *reinterpret_cast<const float4 *>(xb0 + 4 * t);
