@@ -7,8 +7,9 @@
 namespace linmin {
 
 cudaError_t launch_finish_sweep_tu(const LibView &lv, const SolveParams &prm, int sm_count,
-                                   unsigned int *counter, unsigned int *overflow, cudaStream_t stream) {
-    return launch_finish_sweep(lv, prm, sm_count, counter, overflow, stream);
+                                   unsigned int *counter, unsigned int *overflow, const unsigned int *list,
+                                   unsigned int *defer, cudaStream_t stream) {
+    return launch_finish_sweep(lv, prm, sm_count, counter, overflow, list, defer, stream);
 }
 
 }  // namespace linmin

@@ -138,7 +138,11 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) {
 template <int LQ>
 __global__ void __launch_bounds__(384, 1)
 finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter,
-                    unsigned int *__restrict__ overflow /* [0] = count, [1 + i] = pixel */) {
+                    unsigned int *__restrict__ overflow /* [0] = count, [1 + i] = pixel */,
+                    const unsigned int *__restrict__ list /* NULL: all pixels; else the pixels to do, same layout */,
+                    unsigned int *__restrict__ defer /* NULL: run every pixel to its end; else: ONE round per pixel,
+                                                        a pixel whose support has to change is handed on through
+                                                        this list (its repaired support goes to `coeffs`) */) {
     using namespace fs;
     constexpr int NC = 4 * LQ;          // channels per lane
     constexpr int RS = 32 * LQ;         // library row stride (elements)
@@ -188,16 +192,19 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
     // of 4 pixels with neighbouring support sizes: the k-bounded loops of a task then run (almost)
     // without padding (mean of the warp maximum 11.1 -> 8 on config 4).
     int *perm = (int *)((unsigned char *)(At32 + (size_t)RP * RS) + (size_t)(blockDim.x >> 5) * 4 * PIX_BYTES) + warp * 32;
+    const int64_t count = list ? (int64_t)list[0] : prm.N;
     while (true) {
         unsigned int chunk = 0;
         if (lane == 0) chunk = atomicAdd(counter, 1u);
         chunk = __shfl_sync(FULL, chunk, 0);
         const int64_t pbase = (int64_t)chunk * 32;
-        if (pbase >= prm.N) break;
+        if (pbase >= count) break;
+        // my pixel of the chunk (-1: none)
+        const int64_t mypix = (pbase + lane < count) ? (list ? (int64_t)list[1 + pbase + lane] : pbase + lane) : -1;
         {
             int kc = -1;
-            if (pbase + lane < prm.N) {
-                const float *cp = prm.coeffs + (pbase + lane) * R;
+            if (mypix >= 0) {
+                const float *cp = prm.coeffs + mypix * R;
                 kc = 0;
                 if (cvec_ok) {
                     for (int i = 0; i < R; i += 4) {
@@ -221,9 +228,9 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             __syncwarp();
         }
       for (int task = 0; task < 8; ++task) {
-        const int64_t p_raw = pbase + perm[4 * task + g];
-        if (pbase + perm[4 * task] >= prm.N) break;          // sorted: invalid pixels (k = -1) come last
-        const bool valid = p_raw < prm.N;
+        const int64_t p_raw = __shfl_sync(FULL, mypix, perm[4 * task + g]);
+        if (__shfl_sync(FULL, mypix, perm[4 * task]) < 0) break;          // sorted: invalid pixels (k = -1) come last
+        const bool valid = p_raw >= 0;
         const int64_t p = valid ? p_raw : (prm.N - 1);
         float *cout = prm.coeffs + p * R;
         int info = prm.info ? prm.info[p] : 0;
@@ -348,7 +355,8 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
         }
         __syncwarp();
 
-        int pivots = 0, last_added = -1;
+        int pivots = (list && prm.info) ? ((info >> 16) & 0xff) : 0;      // a handed-on pixel keeps its count
+        int last_added = -1;
         unsigned have = 0u;              // endmembers whose b_i = A_i'y is in bE
         double q0 = 0.0, q1 = 0.0, sq = 1.0, rss = 0.0;
 
@@ -695,19 +703,30 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 }
                 __syncwarp();
             }
+            if (defer && st == 0) st = 4;        // one round only: the next one belongs to the repair pass
         }
 
         const bool wr = (st == 1 || st == 2);
+        const bool df = (st == 4);
         if (st == 2) info |= LINMIN_INFO_FINISH_FALLBACK;
         // ---- coefficients (exact zeros off the support), staged in endmember order
-        if (wr) *reinterpret_cast<float4 *>(gs + 4 * t) = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        if (wr || df) *reinterpret_cast<float4 *>(gs + 4 * t) = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         __syncwarp();
         if (wr) {
             if (t < k) gs[i0] = (float)a0;
             if (t + 8 < k) gs[i1] = (float)a1;
         }
+        if (df) {       // the support as it stands now (a member just added sits at 0), kept above the threshold
+            if (t < k) gs[i0] = fmaxf((float)a0, 1.5f * LINMIN_SUPPORT_THRESHOLD);
+            if (t + 8 < k) gs[i1] = fmaxf((float)a1, 1.5f * LINMIN_SUPPORT_THRESHOLD);
+            if (t == 0) {
+                const unsigned slot = atomicAdd(defer, 1u);
+                defer[1 + slot] = (unsigned)p;
+                if (prm.info) prm.info[p] = (info & 0xffff) | ((pivots > 255 ? 255 : pivots) << 16);
+            }
+        }
         __syncwarp();
-        if (wr) {
+        if (wr || df) {
             const float4 o = *reinterpret_cast<const float4 *>(gs + 4 * t);
             if (cvec_ok && 4 * t < R) *reinterpret_cast<float4 *>(cout + 4 * t) = o;
             else {
@@ -805,7 +824,8 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
 
 template <int LQ>
 inline cudaError_t launch_finish_sweep_lq(const LibView &lv, const SolveParams &prm, int sm_count,
-                                          unsigned int *counter, unsigned int *overflow, cudaStream_t stream) {
+                                          unsigned int *counter, unsigned int *overflow, const unsigned int *list,
+                                          unsigned int *defer, cudaStream_t stream) {
     const size_t cta = (fs::cta_bytes(LQ) + 15) & ~(size_t)15;
     const size_t per_warp = 4 * (size_t)fs::PIX_BYTES + 128;     // scratch of 4 pixels + the chunk permutation
     int warps = (int)std::min<size_t>(12, (227 * 1024 - cta) / per_warp);
@@ -816,15 +836,16 @@ inline cudaError_t launch_finish_sweep_lq(const LibView &lv, const SolveParams &
     const int64_t chunks = (prm.N + 31) / 32;
     const int64_t need = (chunks + warps - 1) / warps;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, sm_count));
-    finish_sweep_kernel<LQ><<<grid, warps * 32, smem, stream>>>(lv, prm, counter, overflow);
+    finish_sweep_kernel<LQ><<<grid, warps * 32, smem, stream>>>(lv, prm, counter, overflow, list, defer);
     return cudaGetLastError();
 }
 
-// counter and overflow[0] must be zero (the caller clears them on the stream)
+// counter, overflow[0] and defer[0] must be zero (the caller clears them on the stream)
 inline cudaError_t launch_finish_sweep(const LibView &lv, const SolveParams &prm, int sm_count,
-                                       unsigned int *counter, unsigned int *overflow, cudaStream_t stream) {
-    if (lv.L <= 128) return launch_finish_sweep_lq<4>(lv, prm, sm_count, counter, overflow, stream);
-    return launch_finish_sweep_lq<8>(lv, prm, sm_count, counter, overflow, stream);
+                                       unsigned int *counter, unsigned int *overflow, const unsigned int *list,
+                                       unsigned int *defer, cudaStream_t stream) {
+    if (lv.L <= 128) return launch_finish_sweep_lq<4>(lv, prm, sm_count, counter, overflow, list, defer, stream);
+    return launch_finish_sweep_lq<8>(lv, prm, sm_count, counter, overflow, list, defer, stream);
 }
 
 }  // namespace linmin

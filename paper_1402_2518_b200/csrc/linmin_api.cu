@@ -24,7 +24,8 @@ using namespace linmin;
 namespace linmin {
 // finish_sweep.cu (own translation unit, own register budget)
 cudaError_t launch_finish_sweep_tu(const LibView &lv, const SolveParams &prm, int sm_count,
-                                   unsigned int *counter, unsigned int *overflow, cudaStream_t stream);
+                                   unsigned int *counter, unsigned int *overflow, const unsigned int *list,
+                                   unsigned int *defer, cudaStream_t stream);
 inline bool finish_sweep_supported(int L, int R) { return R <= 32 && L <= 256; }
 }  // namespace linmin
 
@@ -171,15 +172,17 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     if (lib->timing) CK(cudaEventRecord(lib->ev[0], o.stream));
 
     // ---- K1: projection + IPLS
-    // per-call workspace, because one handle may serve several streams: three work counters of the
-    // persistent kernels, then the overflow list of finish_sweep (count + one entry per pixel)
+    // per-call workspace, because one handle may serve several streams: the work counters of the persistent
+    // kernels (8 words), then two pixel lists of finish_sweep (count + one entry per pixel each): the overflow
+    // list (supports above 16) and the repair list (pixels whose support changes after the first round)
     const bool use_f8 = finish_sweep_supported(L, R);
     unsigned int *ws = nullptr;
-    const size_t ws_words = 4 + (use_f8 ? (size_t)N + 1 : 0);
+    const size_t ws_words = 8 + (use_f8 ? 2 * ((size_t)N + 1) : 0);
     CK(staging_alloc((void **)&ws, ws_words * sizeof(unsigned int), o.stream));
     struct Free { unsigned int *p; cudaStream_t s; ~Free() { cudaFreeAsync(p, s); } } free_ws{ws, o.stream};
-    CK(cudaMemsetAsync(ws, 0, std::min<size_t>(5, ws_words) * sizeof(unsigned int), o.stream));
-    unsigned int *counters = ws, *overflow = ws + 4;
+    CK(cudaMemsetAsync(ws, 0, std::min<size_t>(9, ws_words) * sizeof(unsigned int), o.stream));
+    unsigned int *counters = ws, *overflow = ws + 8, *repair = ws + 8 + ((size_t)N + 1);
+    if (use_f8) CK(cudaMemsetAsync(repair, 0, sizeof(unsigned int), o.stream));
     if (R == 32 && ipls_r32_supported(L)) {
         CK(launch_ipls_r32(lv, prm, lib->sm_count, counters, o.stream));
         ++launches;
@@ -203,7 +206,11 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     if (lib->timing) CK(cudaEventRecord(lib->ev[1], o.stream));
     // ---- K2: exact finish + uncertainty + residual
     if (use_f8) {
-        CK(launch_finish_sweep_tu(lv, prm, lib->sm_count, counters + 1, overflow, o.stream));
+        // first round for every pixel (91 % end there), then the others, packed, to their end: a warp's four
+        // pixels share every round, so a repair in the main pass would stall the three that are done
+        CK(launch_finish_sweep_tu(lv, prm, lib->sm_count, counters + 1, overflow, nullptr, repair, o.stream));
+        ++launches;
+        CK(launch_finish_sweep_tu(lv, prm, lib->sm_count, counters + 3, overflow, repair, nullptr, o.stream));
         ++launches;
         // pixels whose support outgrew finish_sweep (none on the synthetic cubes): one-warp-per-pixel kernel
         CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, o.stream));
