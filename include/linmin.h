@@ -95,8 +95,8 @@ typedef struct linmin_opts {
     int32_t constraint;         /* LINMIN_CONSTRAINT_* */
     int32_t weighting;          /* LINMIN_WEIGHTING_* */
     int32_t max_iter;           /* IPLS iteration cap, 1..255; 0 -> 50 */
-    float gap_tol;              /* stop when a'lambda <= gap_tol * scale; 0 -> 1e-8 */
-    float feas_tol;             /* ... and dual/primal residuals <= feas_tol (* scale); 0 -> 1e-6 */
+    float gap_tol;              /* stop when a'lambda <= gap_tol * scale; 0 -> 1e-7 */
+    float feas_tol;             /* ... and dual/primal residuals <= feas_tol (* scale); 0 -> 3e-5 */
     int32_t *info_out;          /* optional int32[N] (device pointer; host pointer for linmin_unmix_host) */
     int32_t deterministic;      /* results never depend on tiling or scheduling; kept for ABI, always on */
     int32_t reserved;

@@ -193,14 +193,16 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
     // without padding (mean of the warp maximum 11.1 -> 8 on config 4).
     int *perm = (int *)((unsigned char *)(At32 + (size_t)RP * RS) + (size_t)(blockDim.x >> 5) * 4 * PIX_BYTES) + warp * 32;
     const int64_t count = list ? (int64_t)list[0] : prm.N;
+    // a short list is dealt out one task (4 pixels) at a time: 32-pixel chunks would leave most warps idle
+    const int csz = (list && count < (int64_t)gridDim.x * (blockDim.x >> 5) * 128) ? 4 : 32;
     while (true) {
         unsigned int chunk = 0;
         if (lane == 0) chunk = atomicAdd(counter, 1u);
         chunk = __shfl_sync(FULL, chunk, 0);
-        const int64_t pbase = (int64_t)chunk * 32;
+        const int64_t pbase = (int64_t)chunk * csz;
         if (pbase >= count) break;
         // my pixel of the chunk (-1: none)
-        const int64_t mypix = (pbase + lane < count) ? (list ? (int64_t)list[1 + pbase + lane] : pbase + lane) : -1;
+        const int64_t mypix = (lane < csz && pbase + lane < count) ? (list ? (int64_t)list[1 + pbase + lane] : pbase + lane) : -1;
         {
             int kc = -1;
             if (mypix >= 0) {
