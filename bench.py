@@ -52,6 +52,14 @@ def flops_model(L, R, it, piv, k):
     return float((proj + ipls).sum()), float((fin + unc + res).sum())
 
 
+def executed_ipls_flops(L, R, it):
+    """What one iteration of the IPLS kernel executes as useful flops: R^3/3 for the factorisation and
+    five triangular solves (5 R^2) -- G a is carried by the Newton identity instead of a mat-vec -- against the
+    R^3/3 + 8 R^2 + 30 R of the SURVEY's model."""
+    it = it.astype(np.float64)
+    return float((2.0 * L * R + it * (R ** 3 / 3.0 + 5.0 * R ** 2)).sum())
+
+
 def gen_cubes(first_cube, n_cubes, Y_out, S_out, threads):
     """Fill Y_out, S_out (numpy views, (n_cubes*CUBE, L)) with cubes first_cube.. of config 4."""
     cfg = CONFIGS["throughput"]
@@ -169,7 +177,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cubes", type=int, default=CONFIGS["throughput"]["cubes"],
                     help="cubes of 131072 pixels per GPU (default 128 = config 4; fewer only for quick checks)")
-    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--sample", type=int, default=None, help="pixels in the cpu_baseline / reference sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -227,6 +235,23 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    def step_shared():
+        linmin.unmix_lib(lib, Yd, Sshared, out=out)
+
+    # second timed mode: ONE shared per-channel sigma[L], the paper's own case (one noise
+    # covariance per image) -- half the input bytes
+    Sshared = Sd[0].clone()
+    for _ in range(max(args.warmup, 3)):
+        step_shared()
+    barrier()
+    evs0, evs1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    evs0.record()
+    for _ in range(args.steps):
+        step_shared()
+    evs1.record()
+    barrier()
+    ms_shared = max_over_ranks(evs0.elapsed_time(evs1) / args.steps, dev)
+
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
@@ -268,16 +293,24 @@ def main():
         except (OSError, ValueError):
             traffic = None
     try:
-        ffma_tf, ffma2_tf = linmin.probe_fp32_peak()
+        from paper_1402_2518_b200.fp32_probe import probe_fp32_peak
+        ffma_tf, ffma2_tf = probe_fp32_peak()
     except Exception:  # report helper only: never fail the bench line on it
         ffma_tf, ffma2_tf = None, None
+    f_exec = executed_ipls_flops(L, R, it)
     roofline = {
         "bound": "alu", "kernel": "projection+IPLS kernel (K1)", "achieved": achieved,
         "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
         "traffic": traffic,
+        "traffic_source": "STORED, not measured by this run: dram bytes per pixel of the ncu --set full capture in "
+                          "profiles/ncu_traffic.json x N",
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no FP32 figure",
         "peak_measured_TFLOPs": {"ffma": ffma_tf, "ffma2": ffma2_tf,
-                                 "how": "linmin_probe_fp32_peak: register-resident independent FMA chains, 8 CTAs x 256 threads per SM"},
+                                 "how": "libfp32probe.so: register-resident independent FMA chains, 8 CTAs x 256 threads per SM"},
+        # the same fraction three ways: SURVEY model / derived peak (the contract), SURVEY model / in-run FFMA2 probe,
+        # executed-flop model (R^3/3 + 5 R^2 per iteration) / derived peak
+        "frac_vs_probe": (achieved / ffma2_tf) if ffma2_tf else None,
+        "frac_executed_flops": f_exec / (ipls_avg * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
         "kernel_ms": {"ipls": ipls_avg, "finish": fin_avg},
         "algorithmic_flops_per_pixel": {"ipls_kernel": f_ipls / N, "finish_kernel": f_fin / N},
         "whole_step": {"achieved": (f_ipls + f_fin) / (ms_step * 1e-3) / 1e12,
@@ -352,6 +385,8 @@ def main():
                        "precompute": "library handle created once outside the timed region (once-per-library step a0)",
                        "arithmetic": "fp32 IPLS; fp64 k x k factor and residual in the finish",
                        "host_generation_s": t_gen},
+            "shared_sigma": {"value": world * N / (ms_shared * 1e-3), "unit": UNIT, "ms_per_step": ms_shared,
+                             "what": "same step with ONE shared sigma[L] (sigma_pixel_stride = 0), device-resident"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
             "cpu_baseline": cpu_baseline, "parity_sample": parity,
         }

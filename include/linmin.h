@@ -33,15 +33,23 @@
  *
  * Device entry points (linmin_unmix, linmin_unmix_lib): every data pointer is a DEVICE pointer on
  * the current CUDA device.  Work is enqueued on opts->stream and the call returns without waiting
- * for it; there is no host round-trip inside the per-pixel iteration.  Argument errors are returned
- * synchronously; asynchronous CUDA errors surface at the next call or stream synchronisation.
+ * for it: no stream synchronisation, no host round-trip, no arithmetic of the method on the host
+ * (both calls can be captured into a CUDA graph).  Argument errors are returned synchronously;
+ * asynchronous CUDA errors surface at the next call or stream synchronisation.
  * Host entry point (linmin_unmix_host): every data pointer is a HOST pointer (pinned memory gives
  * full copy bandwidth); the call stages chunks through the device and returns when outputs are
  * complete.
  *
  * There is no CPU fallback anywhere: without a CUDA device every compute call fails with
- * LINMIN_ERR_CUDA.  No exceptions cross this ABI; no global mutable state; calls on distinct
- * streams / handles are thread-safe.
+ * LINMIN_ERR_CUDA.  No exceptions cross this ABI.  Process-wide state: one staging memory pool per
+ * device (created on first use, guarded by a mutex, see linmin_trim_memory); nothing else.  Calls on
+ * distinct streams, with the same or with different handles, are thread-safe: a solve call reads the
+ * handle and writes only its report fields (launch count, timing events: last caller wins) and its
+ * per-stream "last use" events (under a mutex).
+ *
+ * Defaults that differ from the first draft of this boundary (SURVEY.md 8(b) proposed gap_tol 1e-8,
+ * feas_tol 1e-6): gap_tol 1e-7, feas_tol 3e-5 -- the measured optimum of IPLS + exact finish
+ * together.  Results do not depend on them: every pixel is finished exactly.
  */
 #ifndef LINMIN_H_
 #define LINMIN_H_
@@ -52,7 +60,7 @@
 extern "C" {
 #endif
 
-#define LINMIN_VERSION 100 /* 0.1.0 */
+#define LINMIN_VERSION 200 /* 0.2.0 */
 
 /* status codes: 0 ok, < 0 error, > 0 warning (results valid) */
 #define LINMIN_OK 0
@@ -83,6 +91,7 @@ extern "C" {
 #define LINMIN_INFO_CHOL_REGULARISED 0x08 /* a Newton-matrix pivot was clamped */
 #define LINMIN_INFO_FINISH_FALLBACK 0x10 /* finish hit its pivot/support cap: result feasible, near-optimal, not certified */
 #define LINMIN_INFO_BAD_SIGMA 0x20      /* sigma <= 0 or non-finite: coeff_sigma of the pixel is NaN */
+#define LINMIN_INFO_LIBRARY_NONFINITE 0x40 /* linmin_unmix only: A holds NaN/Inf, every output of the call is NaN */
 #define LINMIN_INFO_ITERATIONS(w) (((w) >> 8) & 0xff)  /* IPLS Newton iterations */
 #define LINMIN_INFO_PIVOTS(w) (((w) >> 16) & 0xff)     /* finish support changes */
 #define LINMIN_INFO_SUPPORT(w) (((w) >> 24) & 0xff)    /* number of non-zero coefficients */
@@ -105,21 +114,31 @@ typedef struct linmin_opts {
 typedef struct linmin_library linmin_library; /* opaque: precomputed per-library data on the device */
 
 /* Once-per-library precompute ("S.S^T"): centred library, Gram
- * matrices in fp32 and fp64.  A is a DEVICE pointer (copied; the caller may free it afterwards).
- * Synchronises the stream once to validate A.  Returns LINMIN_OK, LINMIN_WARN_RANK_DEFICIENT
- * (handle valid) or an error (*lib = NULL).  Only opts->stream is read. */
+ * matrices in fp32 and fp64, and the start-point data of IPLS (inverse of the regularised Gram
+ * matrix) -- all computed by kernels on opts->stream.  A is a DEVICE pointer (copied; the caller may
+ * free it afterwards).  Synchronises the stream ONCE, at the end, to read the device flag that says
+ * whether A is finite.  Returns LINMIN_OK, LINMIN_WARN_RANK_DEFICIENT (handle valid) or an error
+ * (*lib = NULL; LINMIN_ERR_LIBRARY_NONFINITE for NaN/Inf in A).  Only opts->stream is read. */
 int linmin_library_create(const float *A, int32_t L, int32_t R, const linmin_opts *opts,
                           linmin_library **lib);
 
-/* Frees the handle's device memory (stream-ordered after all work enqueued with it). NULL is a no-op. */
+/* Frees the handle's device memory, stream-ordered on the creation stream AFTER the last work enqueued
+ * with the handle on any stream (the library records an event per stream it served and the creation
+ * stream waits for them).  Exception: work captured into a CUDA graph is not tracked -- keep the handle
+ * alive as long as the graph may be launched.  NULL is a no-op. */
 void linmin_library_destroy(linmin_library *lib);
 
-/* Unmix N spectra against a precomputed library.  Device pointers.  N == 0 is a no-op. */
+/* Unmix N spectra against a precomputed library.  Device pointers on the handle's device (another
+ * current device -> LINMIN_ERR_INVALID_ARGUMENT).  N == 0 is a no-op; N >= 2^32 ->
+ * LINMIN_ERR_UNSUPPORTED_SIZE.  Enqueues and returns. */
 int linmin_unmix_lib(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
                      const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out,
                      float *resid_out);
 
-/* One-shot form: linmin_library_create + linmin_unmix_lib + linmin_library_destroy. Device pointers. */
+/* One-shot form: precompute + solve + release, all enqueued on opts->stream; returns without waiting.
+ * Device pointers.  Since nothing is read back, a non-finite library is reported through the OUTPUTS:
+ * all of them NaN, every info word = LINMIN_INFO_LIBRARY_NONFINITE (linmin_library_create reports
+ * it as a status instead). */
 int linmin_unmix(const float *A, const float *Y, const float *sigma, int64_t N, int32_t L, int32_t R,
                  const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out, float *resid_out);
 
@@ -140,12 +159,6 @@ int linmin_library_last_launches(const linmin_library *lib);
  * timing is disabled or no call was made.  Not thread-safe per handle. */
 int linmin_library_enable_timing(linmin_library *lib, int enable);
 int linmin_library_last_timing(const linmin_library *lib, float *ipls_ms, float *finish_ms);
-
-/* Report helper for the roofline denominator (bench.py): measures what the FP32 FMA pipe of the current
- * device sustains, in TFLOP/s (2 flops per FMA), with register-resident independent FMA chains: scalar
- * FFMA in *ffma_tflops, packed FFMA2 (fma.rn.f32x2) in *ffma2_tflops (host pointers).  Synchronous; runs
- * a few milliseconds of work on `stream` (a cudaStream_t, NULL = default stream).  Not on the hot path. */
-int linmin_probe_fp32_peak(void *stream, double *ffma_tflops, double *ffma2_tflops);
 
 /* Staging memory (per-call workspaces of linmin_unmix_lib, the device buffers of linmin_unmix_host) is taken
  * from a memory pool the library owns, one per device, and kept between calls.  linmin_trim_memory() returns

@@ -25,7 +25,8 @@ struct LibView {
     const float *c;     // L
     const float *Gc;    // R x R fp32, Gc = Ac' Ac accumulated in fp64 (drives IPLS)
     const double *G64;  // R x R fp64, G = A' A (uncentred, exact data; drives the finish)
-    float gdmax;        // max_i Gc[i][i]
+    const float *scal;  // device scalars of the precompute: [0] gdmax = max_i Gc[i][i] (1 if that is 0), [1] sum of Giq
+    const int *flags;   // device word: bit 0 = the library holds a non-finite value (every kernel then returns at once)
     const float *Gi;    // R x R fp32, (Gc + 1e-4 gdmax I)^-1 (start point of IPLS: regularised sum-constrained LS)
     const float *Giq;   // R, row sums of Gi
 };
@@ -67,6 +68,67 @@ __device__ __forceinline__ float warp_min(float v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
     return v;
+}
+
+// ---- reductions over a group of W consecutive lanes (W = 4 or 8 lanes cooperate on one pixel)
+template <int W> __device__ __forceinline__ float group_sum(float v) {
+#pragma unroll
+    for (int o = 1; o < W; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+template <int W> __device__ __forceinline__ double group_sum(double v) {
+#pragma unroll
+    for (int o = 1; o < W; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+template <int W> __device__ __forceinline__ float group_min(float v) {
+#pragma unroll
+    for (int o = 1; o < W; o <<= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+template <int W> __device__ __forceinline__ double group_min(double v) {
+#pragma unroll
+    for (int o = 1; o < W; o <<= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+template <int W> __device__ __forceinline__ float group_max(float v) {
+#pragma unroll
+    for (int o = 1; o < W; o <<= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+template <int W> __device__ __forceinline__ unsigned group_or(unsigned v) {
+#pragma unroll
+    for (int o = 1; o < W; o <<= 1) v |= __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ float rcp_approx(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+// ---- packed fp32 arithmetic (sm_100 FFMA2 / FMUL2: the FP32 peak of this part is an FFMA2 peak)
+__device__ __forceinline__ unsigned long long pk2(float2 v) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(v.x), "f"(v.y));
+    return r;
+}
+__device__ __forceinline__ float2 upk2(unsigned long long v) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+// a * b + c on both halves; the scalar form broadcasts a
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pk2(a)), "l"(pk2(b)), "l"(pk2(c)));
+    return upk2(d);
+}
+__device__ __forceinline__ float2 fma2(float a, float2 b, float2 c) { return fma2(make_float2(a, a), b, c); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) {
+    unsigned long long d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk2(a)), "l"(pk2(b)));
+    return upk2(d);
 }
 
 }  // namespace linmin

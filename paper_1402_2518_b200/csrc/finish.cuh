@@ -38,6 +38,7 @@ __host__ __device__ inline size_t finish_warp_bytes(int L, int R, int KMAX) {
 // state[i]: 0 free, 1 in F, 2 blocked (rejected as rank-deficient or degenerate tie)
 __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams prm, int KMAX) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (lib.flags[0] & 1) return;
     const int L = lib.L, R = lib.R;
     const int warps = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned char *basep = smem_raw + (size_t)warp * ((finish_warp_bytes(L, R, KMAX) + 15) & ~(size_t)15);

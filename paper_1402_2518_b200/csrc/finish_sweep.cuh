@@ -45,42 +45,12 @@ __host__ __device__ inline size_t cta_bytes(int LQ) {
     return (size_t)RP * GS * 8 + (size_t)RP * 32 * LQ * 4;
 }
 
-__device__ __forceinline__ double gsum(double v) {
-    v += __shfl_xor_sync(FULL, v, 1);
-    v += __shfl_xor_sync(FULL, v, 2);
-    v += __shfl_xor_sync(FULL, v, 4);
-    return v;
-}
-__device__ __forceinline__ float gsum(float v) {
-    v += __shfl_xor_sync(FULL, v, 1);
-    v += __shfl_xor_sync(FULL, v, 2);
-    v += __shfl_xor_sync(FULL, v, 4);
-    return v;
-}
-__device__ __forceinline__ double gmin(double v) {
-    v = fmin(v, __shfl_xor_sync(FULL, v, 1));
-    v = fmin(v, __shfl_xor_sync(FULL, v, 2));
-    v = fmin(v, __shfl_xor_sync(FULL, v, 4));
-    return v;
-}
-__device__ __forceinline__ float gminf(float v) {
-    v = fminf(v, __shfl_xor_sync(FULL, v, 1));
-    v = fminf(v, __shfl_xor_sync(FULL, v, 2));
-    v = fminf(v, __shfl_xor_sync(FULL, v, 4));
-    return v;
-}
-__device__ __forceinline__ float gmaxf(float v) {
-    v = fmaxf(v, __shfl_xor_sync(FULL, v, 1));
-    v = fmaxf(v, __shfl_xor_sync(FULL, v, 2));
-    v = fmaxf(v, __shfl_xor_sync(FULL, v, 4));
-    return v;
-}
-__device__ __forceinline__ unsigned gor(unsigned v) {
-    v |= __shfl_xor_sync(FULL, v, 1);
-    v |= __shfl_xor_sync(FULL, v, 2);
-    v |= __shfl_xor_sync(FULL, v, 4);
-    return v;
-}
+__device__ __forceinline__ double gsum(double v) { return group_sum<8>(v); }   // over the 8 lanes of a pixel
+__device__ __forceinline__ float gsum(float v) { return group_sum<8>(v); }
+__device__ __forceinline__ double gmin(double v) { return group_min<8>(v); }
+__device__ __forceinline__ float gminf(float v) { return group_min<8>(v); }
+__device__ __forceinline__ float gmaxf(float v) { return group_max<8>(v); }
+__device__ __forceinline__ unsigned gor(unsigned v) { return group_or<8>(v); }
 __device__ __forceinline__ int wmax(int v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(FULL, v, o));
@@ -109,29 +79,6 @@ __device__ __forceinline__ double rcp_d(double x) {
     e = fma(-x, p, 1.0);
     return fma(p, e, p);
 }
-// packed fp32 arithmetic (sm_100 FFMA2 / FMUL2)
-__device__ __forceinline__ unsigned long long pk2(float2 v) {
-    unsigned long long r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(v.x), "f"(v.y));
-    return r;
-}
-__device__ __forceinline__ float2 upk2(unsigned long long v) {
-    float2 r;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
-    return r;
-}
-__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
-    unsigned long long d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pk2(a)), "l"(pk2(b)), "l"(pk2(c)));
-    return upk2(d);
-}
-__device__ __forceinline__ float2 fma2(float a, float2 b, float2 c) { return fma2(make_float2(a, a), b, c); }
-__device__ __forceinline__ float2 mul2(float2 a, float2 b) {
-    unsigned long long d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk2(a)), "l"(pk2(b)));
-    return upk2(d);
-}
-
 }  // namespace fs
 
 // LQ = float4 chunks of the spectrum per lane: L <= 32 LQ
@@ -148,6 +95,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
     constexpr int RS = 32 * LQ;         // library row stride (elements)
     constexpr int IT = (LQ <= 4) ? 4 : 2;   // J rows per tile
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (lib.flags[0] & 1) return;
     const int L = lib.L, R = lib.R;
     double *G64s = (double *)smem_raw;                                    // [RP][GS]
     float *At32 = (float *)(smem_raw + (size_t)RP * GS * 8);              // [RP][32 LQ]: library rows, fp32 (widened on the fly:
@@ -469,6 +417,8 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             bool skip = !act;
             bool fell = false;      // this round ended in the fallback state: the residual is still due
             if (__any_sync(FULL, act && rej >= 0)) {       // warp-uniform and rare (duplicate or collinear members)
+                const int rj = rej >= 0 ? rej : 0;
+                const int irej = __shfl_sync(FULL, (rj < 8) ? i0 : i1, rj & 7, 8);     // endmember of the rejected member
                 if (act && rej >= 0) {
                     // A_F lost rank at member `rej` (R9): drop it, block it, stay at the same point
                     skip = true;
@@ -488,13 +438,17 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 }
                 const double s = gsum(a0 + a1);
                 if (act && rej >= 0) {
-                    if (k == 0 || pivots > max_pivots) {
+                    if (k == 0) {
+                        // the only member was rejected (a zero endmember): stay on the simplex with it, uncertified
+                        k = 1; i0 = (t == 0) ? irej : 0; a0 = (t == 0) ? 1.0 : 0.0;
+                        if (t == 0) { idx[0] = irej; aFs[0] = 1.0; state[irej] = 1; }
                         st = 2; fell = true;
                     } else {
                         const double rs = rcp_d(s);
                         a0 *= rs; a1 *= rs;
                         if (t < k) aFs[t] = a0;
                         if (t + 8 < k) aFs[t + 8] = a1;
+                        if (pivots > max_pivots) { st = 2; fell = true; }
                     }
                 }
                 __syncwarp();

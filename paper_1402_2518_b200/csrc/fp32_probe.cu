@@ -1,11 +1,11 @@
-// probe.cuh -- FP32 FMA-pipe probe for the roofline denominator (report helper, not on the hot path).
+// fp32_probe.cu -- FP32 FMA-pipe probe for the roofline denominator: a bench-side helper built into its own
+// library (libfp32probe.so), NOT part of liblinmin.so or of include/linmin.h.
 // MEASURED_PEAKS.json carries HBM and bf16 tensor figures only; the path here is bound by plain FP32
-// arithmetic, so the bench measures what the FMA pipe sustains: every thread runs
+// arithmetic, so bench.py measures what the FMA pipe sustains: every thread runs
 // independent dependent-free FMA chains from registers, as scalar FFMA and as packed FFMA2.
-#pragma once
-#include "common.cuh"
+#include <cuda_runtime.h>
 
-namespace linmin {
+namespace {
 
 template <bool PACKED>
 __global__ void __launch_bounds__(256) fp32_probe_kernel(float *sink, int iters, float seed) {
@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(256) fp32_probe_kernel(float *sink, int iters,
 }
 
 // Returns TFLOP/s (2 flops per FMA) of scalar FFMA and of packed FFMA2 streams on the device of `stream`.
-inline cudaError_t probe_fp32(int sm_count, cudaStream_t stream, double *ffma_tflops, double *ffma2_tflops) {
+cudaError_t probe_fp32(int sm_count, cudaStream_t stream, double *ffma_tflops, double *ffma2_tflops) {
     float *sink = nullptr;
     cudaError_t e = cudaMalloc((void **)&sink, sizeof(float) * 256);
     if (e != cudaSuccess) return e;
@@ -68,4 +68,15 @@ inline cudaError_t probe_fp32(int sm_count, cudaStream_t stream, double *ffma_tf
     return e;
 }
 
-}  // namespace linmin
+}  // namespace
+
+// host pointers; synchronous; a few milliseconds of work on `stream` (a cudaStream_t, NULL = default stream).
+// Returns 0 or a cudaError_t.
+extern "C" int fp32_probe_peak(void *stream, double *ffma_tflops, double *ffma2_tflops) {
+    if (!ffma_tflops || !ffma2_tflops) return (int)cudaErrorInvalidValue;
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = probe_fp32(sms, (cudaStream_t)stream, ffma_tflops, ffma2_tflops);
+    return (int)e;
+}

@@ -278,6 +278,8 @@ template <int TEAM>
 __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolveParams prm) {
     using Ops = TeamOps<TEAM>;
     extern __shared__ __align__(16) float smem[];
+    if (lib.flags[0] & 1) return;      // non-finite library: the caller is told (status or poisoned outputs)
+    const float gdmax = lib.scal[0];
     const int L = lib.L, R = lib.R;
     const int teams_per_cta = blockDim.x / TEAM;
     const int team = threadIdx.x / TEAM;
@@ -316,7 +318,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
             bmax = fmaxf(bmax, fabsf(s));
         }
         bmax = Ops::max(bmax, red);
-        const float sc = fmaxf(bmax, 1e-3f * lib.gdmax);
+        const float sc = fmaxf(bmax, 1e-3f * gdmax);
         // ---- start (Mehrotra's heuristic, as in ipls_r32.cuh): the sum-constrained LS point of the regularised
         //      problem, x = Gi b - q (1'Gi b - 1)/(1'q), its reduced gradient as multipliers, both shifted inside
         float nu, lam0;
@@ -362,7 +364,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
             sa = Ops::sum(sa, red); lam0 = Ops::max(lm, red);
             const float rsa = 1.0f / sa;
             const bool ok = (lam0 > 0.0f) && isfinite(lam0) && isfinite(sa) && isfinite(rsa);
-            if (!ok) { lam0 = fmaxf(bmax, 1e-3f * lib.gdmax); nu = 0.0f; }
+            if (!ok) { lam0 = fmaxf(bmax, 1e-3f * gdmax); nu = 0.0f; }
             for (int i = t; i < R; i += TEAM) {
                 if (ok) {
                     a[i] *= rsa;
@@ -406,7 +408,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
                         Mp[ipls_rowoff(i) + k] = m;
                     }
                 Ops::sync();
-                regularised = warp_cholesky_rm(Mp, dinv, R, 1e-12f * lib.gdmax);
+                regularised = warp_cholesky_rm(Mp, dinv, R, 1e-12f * gdmax);
             } else {
                 for (int j = 0; j < R; ++j)
                     for (int i = j + t; i < R; i += TEAM) {
@@ -415,7 +417,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
                         Mp[cm(R, i, j)] = m;
                     }
                 Ops::sync();
-                regularised = team_cholesky<TEAM, float>(Mp, dinv, R, 1e-12f * lib.gdmax);
+                regularised = team_cholesky<TEAM, float>(Mp, dinv, R, 1e-12f * gdmax);
             }
             if (regularised) flags |= LINMIN_INFO_CHOL_REGULARISED;
             // ---- predictor

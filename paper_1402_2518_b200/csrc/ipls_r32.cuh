@@ -32,17 +32,6 @@
 
 namespace linmin {
 
-#ifdef IPLS_PHASE_PROF
-__device__ unsigned long long g_phase[16];
-#define PH_DECL long long ph_t = clock64(); long long ph_acc[10] = {0,0,0,0,0,0,0,0,0,0};
-#define PH(i) { long long n__ = clock64(); ph_acc[i] += n__ - ph_t; ph_t = n__; }
-#define PH_FLUSH if (lane == 0) { for (int i__ = 0; i__ < 10; ++i__) atomicAdd(&g_phase[i__], (unsigned long long)ph_acc[i__]); }
-#else
-#define PH_DECL
-#define PH(i)
-#define PH_FLUSH
-#endif
-
 namespace r32 {
 
 constexpr int R = 32;
@@ -56,47 +45,9 @@ constexpr int PIXF = 584;      // fixed floats per pixel (576 used; 584 = 8 mod 
 constexpr int WARPS = 8;      // warps per CTA, one CTA per SM
 constexpr unsigned FULL = 0xffffffffu;
 
-__device__ __forceinline__ float rcp_approx(float x) {
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-__device__ __forceinline__ unsigned long long pk2(float2 v) {
-    unsigned long long r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(v.x), "f"(v.y));
-    return r;
-}
-__device__ __forceinline__ float2 upk2(unsigned long long v) {
-    float2 r;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
-    return r;
-}
-// packed FMA (sm_100 FFMA2): a * b + c on both halves; the scalar form broadcasts a
-__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
-    unsigned long long d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pk2(a)), "l"(pk2(b)), "l"(pk2(c)));
-    return upk2(d);
-}
-__device__ __forceinline__ float2 fma2(float a, float2 b, float2 c) { return fma2(make_float2(a, a), b, c); }
-
-__device__ __forceinline__ float gsum(float v) {   // sum over the 8 lanes of a pixel group
-    v += __shfl_xor_sync(FULL, v, 1);
-    v += __shfl_xor_sync(FULL, v, 2);
-    v += __shfl_xor_sync(FULL, v, 4);
-    return v;
-}
-__device__ __forceinline__ float gmin(float v) {
-    v = fminf(v, __shfl_xor_sync(FULL, v, 1));
-    v = fminf(v, __shfl_xor_sync(FULL, v, 2));
-    v = fminf(v, __shfl_xor_sync(FULL, v, 4));
-    return v;
-}
-__device__ __forceinline__ float gmax(float v) {
-    v = fmaxf(v, __shfl_xor_sync(FULL, v, 1));
-    v = fmaxf(v, __shfl_xor_sync(FULL, v, 2));
-    v = fmaxf(v, __shfl_xor_sync(FULL, v, 4));
-    return v;
-}
+__device__ __forceinline__ float gsum(float v) { return group_sum<8>(v); }   // over the 8 lanes of a pixel
+__device__ __forceinline__ float gmin(float v) { return group_min<8>(v); }
+__device__ __forceinline__ float gmax(float v) { return group_max<8>(v); }
 
 // shared-memory footprint in floats
 __host__ __device__ inline int lpad(int L) { return (L + 3) & ~3; }
@@ -186,6 +137,7 @@ __global__ void __launch_bounds__(r32::WARPS * 32, 1)
 ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter) {
     using namespace r32;
     extern __shared__ __align__(16) float smem[];
+    if (lib.flags[0] & 1) return;      // non-finite library: the caller is told (status or poisoned outputs)
     const int L = lib.L;
     const int Lp = lpad(L);
     float *Gp = smem;                        // [32][GST]
@@ -229,7 +181,7 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
     }
     __syncthreads();
 
-    const float gdmax = lib.gdmax;
+    const float gdmax = lib.scal[0];
     const float tau = 0.995f;
     const float pivot_floor = 1e-12f * gdmax;
     // one-hot pairs of my position inside a diagonal block: adds lambda/a to the diagonal with FFMA2
@@ -256,13 +208,11 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
-    PH_DECL
     unsigned int grp = __shfl_sync(FULL, take_ticket(), 0);
     unsigned int grp_next = __shfl_sync(FULL, take_ticket(), 0);
     prefetch(grp, yb0);
     int par = 0;
     while (true) {
-        PH(8)
         const int64_t p0 = (int64_t)grp * 4;
         if (p0 >= prm.N) break;
         const bool valid = (p0 + g) < prm.N;
@@ -394,8 +344,6 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         }
         int iters = 0, flags = bad ? LINMIN_INFO_NONFINITE_INPUT : 0;
         bool done = false;
-
-        PH(7)
         for (int it = 0;; ++it) {
             // ---- rows of M (lower part) from G.  G a is not recomputed: the Newton system gives
             //      G da = (r1 - dnu 1) - d o da row by row, so G a is carried along with a (no exchange of a,
@@ -410,7 +358,6 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                     m2[s][2 * c + 1] = make_float2(g4.z, g4.w);
                 }
             }
-            PH(0)
             // ---- residuals and stopping rule (per pixel group)
             float rdm = 0.0f, sa = 0.0f, gp = 0.0f;
 #pragma unroll
@@ -432,8 +379,6 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             if (__all_sync(FULL, done)) break;
             if (!done) ++iters;
             const float mu = gp * (1.0f / 32.0f);
-
-            PH(1)
             // ---- M = G + diag(lambda / a)
             float ainv[4], d[4], dinv[4];
 #pragma unroll
@@ -563,7 +508,6 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                 }
             }
 #undef L4C
-            PH(2)
             {   // k = 31: only the last pivot (its owner has it) -- nothing left to update
                 float piv = m2[3][15].y;
                 if (t == 7 && !(piv > pivot_floor)) { piv = pivot_floor; clamped = true; }
@@ -577,7 +521,6 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             TINV_ROWS(3)
 #undef TINV_STORE
 #undef TINV_ROWS
-            PH(3)
             // ---- predictor: M^-1 = L^-T D^-1 L^-1; nu eliminated through L^-1 1
             float sww = 0.0f, swz = 0.0f;
 #pragma unroll
@@ -609,7 +552,6 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             mua = gsum(mua) * (1.0f / 32.0f);
             float sg = mua / mu;
             sg = fminf(1.0f, fmaxf(0.0f, sg * sg * sg));
-            PH(4)
             // ---- corrector
             float cc[4], r1[4];
 #pragma unroll
@@ -618,7 +560,6 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                 r1[s] = fmaf(cc[s], ainv[s], -w[s]);
             }
             forward_subst_blk(m2, ti, r1, agb, t);
-            PH(5)
             swz = 0.0f;
 #pragma unroll
             for (int s = 0; s < 4; ++s) swz = fmaf(rr[s].x * dinv[s], r1[s], swz);
@@ -645,7 +586,6 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
                 lam[s] = fmaxf(fmaf(ad, dl[s], lam[s]), 1e-18f * lam0);
             }
             nu = fmaf(ad, dnu, nu);
-            PH(6)
         }
 
         // ---- store the iterate (coalesced: 8 lanes x float4 = one 128 B row) and the info word
@@ -663,8 +603,6 @@ ipls_r32_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
         grp_next = __shfl_sync(FULL, ticket, 0);
         par ^= 1;
     }
-    PH(8)
-    PH_FLUSH
 }
 #undef LM_COL
 

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -17,7 +18,6 @@
 #include "ipls_generic.cuh"
 #include "ipls_r32.cuh"
 #include "precompute.cuh"
-#include "probe.cuh"
 
 using namespace linmin;
 
@@ -35,12 +35,22 @@ struct linmin_library {
     int sm_count = 0;
     cudaStream_t stream = nullptr;   // stream the handle was created on (frees are ordered on it)
     float *A = nullptr, *At = nullptr, *Ac = nullptr, *c = nullptr, *Gc = nullptr, *Gi = nullptr, *Giq = nullptr;
-    double *G64 = nullptr;
-    float gdmax = 0.0f;
-    mutable int last_launches = 0;
+    float *scal = nullptr;           // device scalars: gdmax, sum of Giq
+    int *flags = nullptr;            // device word: bit 0 = non-finite library
+    double *G64 = nullptr, *W64 = nullptr;
+    // report fields and the last-use events are the only state a solve call writes; the handle is otherwise
+    // immutable after creation (hence `const linmin_library *` in linmin_unmix_lib)
+    mutable std::atomic<int> last_launches{0};
     bool timing = false;
-    mutable bool timed = false;
+    mutable std::atomic<bool> timed{false};
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    // last use per stream: linmin_library_destroy orders its frees after the work of EVERY stream the handle served
+    static constexpr int MAX_USE = 16;
+    mutable std::mutex use_mu;
+    mutable cudaStream_t use_stream[MAX_USE] = {};
+    mutable cudaEvent_t use_event[MAX_USE] = {};
+    mutable int n_use = 0;
+    mutable bool use_overflow = false;   // more streams than slots: destroy synchronises the device instead
 };
 
 namespace {
@@ -90,7 +100,6 @@ int cuda_status(cudaError_t e) {
         cudaError_t e__ = (call);                  \
         if (e__ != cudaSuccess) {                  \
             (void)cudaGetLastError();              \
-            if (getenv("LINMIN_DEBUG")) fprintf(stderr, "linmin: %s at %s:%d\n", cudaGetErrorString(e__), __FILE__, __LINE__); \
             return cuda_status(e__);               \
         }                                          \
     } while (0)
@@ -136,13 +145,14 @@ int resolve_opts(const linmin_opts *o, int L, Resolved *r) {
 int check_sizes(int64_t N, int L, int R) {
     if (N < 0 || L < 1 || R < 1) return LINMIN_ERR_INVALID_ARGUMENT;
     if (R > LINMIN_MAX_R || L > LINMIN_MAX_L) return LINMIN_ERR_UNSUPPORTED_SIZE;
+    if (N >= ((int64_t)1 << 32)) return LINMIN_ERR_UNSUPPORTED_SIZE;   // pixel lists and work tickets are 32-bit
     return LINMIN_OK;
 }
 
 LibView view_of(const linmin_library *lib) {
     LibView v;
     v.L = lib->L; v.R = lib->R; v.A = lib->A; v.At = lib->At; v.Ac = lib->Ac; v.c = lib->c; v.Gc = lib->Gc;
-    v.G64 = lib->G64; v.gdmax = lib->gdmax; v.Gi = lib->Gi; v.Giq = lib->Giq;
+    v.G64 = lib->G64; v.scal = lib->scal; v.flags = lib->flags; v.Gi = lib->Gi; v.Giq = lib->Giq;
     return v;
 }
 
@@ -157,6 +167,26 @@ int persistent_grid(K kernel, int block, size_t smem, int sm_count, int64_t work
     int64_t need = (work_items + items_per_cta - 1) / items_per_cta;
     int64_t cap = (int64_t)sm_count * occ;
     return (int)std::max<int64_t>(1, std::min(need, cap));
+}
+
+// Records "the handle was last used on `stream` now" (one event per stream the handle has served); skipped while
+// the stream is being captured into a CUDA graph (the graph's owner then keeps the handle alive, include/linmin.h).
+void note_use(const linmin_library *lib, cudaStream_t stream) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess) { (void)cudaGetLastError(); return; }
+    if (cs != cudaStreamCaptureStatusNone) return;
+    if (stream == lib->stream) return;            // frees are enqueued on that stream anyway
+    std::lock_guard<std::mutex> lk(lib->use_mu);
+    int slot = -1;
+    for (int i = 0; i < lib->n_use; ++i) if (lib->use_stream[i] == stream) slot = i;
+    if (slot < 0) {
+        if (lib->n_use == linmin_library::MAX_USE) { lib->use_overflow = true; return; }
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) { (void)cudaGetLastError(); lib->use_overflow = true; return; }
+        slot = lib->n_use++;
+        lib->use_stream[slot] = stream; lib->use_event[slot] = e;
+    }
+    if (cudaEventRecord(lib->use_event[slot], stream) != cudaSuccess) { (void)cudaGetLastError(); lib->use_overflow = true; }
 }
 
 int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
@@ -230,12 +260,16 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
         CK(cudaGetLastError());
         ++launches;
     }
-    if (lib->timing) { CK(cudaEventRecord(lib->ev[2], o.stream)); lib->timed = true; }
-    lib->last_launches = launches;
+    if (lib->timing) { CK(cudaEventRecord(lib->ev[2], o.stream)); lib->timed.store(true); }
+    lib->last_launches.store(launches);
+    note_use(lib, o.stream);
     return LINMIN_OK;
 }
 
-int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool A_on_host,
+// Once-per-library precompute, all of it on the device and enqueued on `stream`: copy of A,
+// centred library, transposed copy, Gram matrices, start-point data.  No host round trip; `wait_check` adds the
+// ONE synchronisation linmin_library_create documents (to return LINMIN_ERR_LIBRARY_NONFINITE).
+int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool A_on_host, bool wait_check,
                         linmin_library **out) {
     *out = nullptr;
     int dev = 0;
@@ -243,12 +277,7 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
     linmin_library *lib = new (std::nothrow) linmin_library();
     if (!lib) return LINMIN_ERR_OUT_OF_MEMORY;
     lib->L = L; lib->R = R; lib->device = dev; lib->stream = stream;
-    int rc = LINMIN_OK;
-    int *flags = nullptr;
-    std::vector<float> hG((size_t)R * R);
-    int hflags = 0;
     auto fail = [&](int code) {
-        if (flags) cudaFreeAsync(flags, stream);
         linmin_library_destroy(lib);
         return code;
     };
@@ -264,75 +293,35 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
     CKF(cudaMallocAsync((void **)&lib->Ac, LR * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->c, (size_t)L * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->Gc, RR * sizeof(float), stream));
+    CKF(cudaMallocAsync((void **)&lib->Gi, RR * sizeof(float), stream));
+    CKF(cudaMallocAsync((void **)&lib->Giq, (size_t)R * sizeof(float), stream));
+    CKF(cudaMallocAsync((void **)&lib->scal, 4 * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->G64, RR * sizeof(double), stream));
-    CKF(cudaMallocAsync((void **)&flags, sizeof(int), stream));
-    CKF(cudaMemsetAsync(flags, 0, sizeof(int), stream));
+    CKF(cudaMallocAsync((void **)&lib->W64, RR * sizeof(double), stream));
+    CKF(cudaMallocAsync((void **)&lib->flags, sizeof(int), stream));
+    CKF(cudaMemsetAsync(lib->flags, 0, sizeof(int), stream));
     CKF(cudaMemcpyAsync(lib->A, A, LR * sizeof(float), A_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, stream));
     {
         int block = 256, grid = (L * 32 + block - 1) / block;
-        center_library_kernel<<<grid, block, 0, stream>>>(lib->A, L, R, lib->Ac, lib->c, flags);
+        center_library_kernel<<<grid, block, 0, stream>>>(lib->A, L, R, lib->Ac, lib->c, lib->flags);
         CKF(cudaGetLastError());
         transpose_library_kernel<<<(int)((LR + block - 1) / block), block, 0, stream>>>(lib->A, L, R, lib->At);
         CKF(cudaGetLastError());
         grid = (int)((RR + block - 1) / block);
         gram_kernel<<<grid, block, 0, stream>>>(lib->A, lib->Ac, L, R, lib->G64, lib->Gc);
         CKF(cudaGetLastError());
+        // start point data of IPLS: inverse of the regularised centred Gram matrix, its row sums, gdmax
+        start_data_kernel<<<1, 1024, 0, stream>>>(lib->Gc, R, lib->W64, lib->Gi, lib->Giq, lib->scal);
+        CKF(cudaGetLastError());
     }
-    CKF(cudaMemcpyAsync(hG.data(), lib->Gc, RR * sizeof(float), cudaMemcpyDeviceToHost, stream));
-    CKF(cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, stream));
-    CKF(cudaStreamSynchronize(stream));
-    cudaFreeAsync(flags, stream);
-    flags = nullptr;
-    if (hflags & 1) return fail(LINMIN_ERR_LIBRARY_NONFINITE);
-    float gd = 0.0f;
-    for (int i = 0; i < R; ++i) gd = std::max(gd, hG[(size_t)i * R + i]);
-    if (!(gd > 0.0f)) gd = 1.0f;   // all endmembers identical: any point of the simplex is optimal
-    lib->gdmax = gd;
-    {   // start point data of IPLS: inverse of the regularised centred Gram matrix (fp64 Gauss-Jordan with
-        // partial pivoting on the host, once per library) and its row sums
-        const double delta = 1e-4 * (double)gd;
-        std::vector<double> M((size_t)R * 2 * R, 0.0);
-        for (int i = 0; i < R; ++i) {
-            for (int j = 0; j < R; ++j) M[(size_t)i * 2 * R + j] = (double)hG[(size_t)i * R + j];
-            M[(size_t)i * 2 * R + i] += delta;
-            M[(size_t)i * 2 * R + R + i] = 1.0;
-        }
-        for (int j = 0; j < R; ++j) {
-            int piv = j;
-            for (int i = j + 1; i < R; ++i)
-                if (std::fabs(M[(size_t)i * 2 * R + j]) > std::fabs(M[(size_t)piv * 2 * R + j])) piv = i;
-            if (piv != j)
-                for (int c2 = 0; c2 < 2 * R; ++c2) std::swap(M[(size_t)j * 2 * R + c2], M[(size_t)piv * 2 * R + c2]);
-            double d = M[(size_t)j * 2 * R + j];
-            if (!(std::fabs(d) > 0.0)) d = delta;
-            const double pinv = 1.0 / d;
-            for (int c2 = 0; c2 < 2 * R; ++c2) M[(size_t)j * 2 * R + c2] *= pinv;
-            for (int i = 0; i < R; ++i) {
-                if (i == j) continue;
-                const double f = M[(size_t)i * 2 * R + j];
-                if (f == 0.0) continue;
-                for (int c2 = 0; c2 < 2 * R; ++c2) M[(size_t)i * 2 * R + c2] -= f * M[(size_t)j * 2 * R + c2];
-            }
-        }
-        std::vector<float> hGi(RR), hq(R);
-        for (int i = 0; i < R; ++i) {
-            double q = 0.0;
-            for (int j = 0; j < R; ++j) {
-                const double v = 0.5 * (M[(size_t)i * 2 * R + R + j] + M[(size_t)j * 2 * R + R + i]);
-                hGi[(size_t)i * R + j] = (float)v;
-                q += v;
-            }
-            hq[i] = (float)q;
-        }
-        CKF(cudaMallocAsync((void **)&lib->Gi, RR * sizeof(float), stream));
-        CKF(cudaMallocAsync((void **)&lib->Giq, (size_t)R * sizeof(float), stream));
-        CKF(cudaMemcpyAsync(lib->Gi, hGi.data(), RR * sizeof(float), cudaMemcpyHostToDevice, stream));
-        CKF(cudaMemcpyAsync(lib->Giq, hq.data(), (size_t)R * sizeof(float), cudaMemcpyHostToDevice, stream));
+    if (wait_check) {
+        int hflags = 0;
+        CKF(cudaMemcpyAsync(&hflags, lib->flags, sizeof(int), cudaMemcpyDeviceToHost, stream));
         CKF(cudaStreamSynchronize(stream));
+        if (hflags & 1) return fail(LINMIN_ERR_LIBRARY_NONFINITE);
     }
-    if (R > L) rc = LINMIN_WARN_RANK_DEFICIENT;
     *out = lib;
-    return rc;
+    return (R > L) ? LINMIN_WARN_RANK_DEFICIENT : LINMIN_OK;
 #undef CKF
 }
 
@@ -340,29 +329,12 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
 
 extern "C" {
 
-#ifdef IPLS_PHASE_PROF
-int linmin_debug_phases(unsigned long long *out16, int reset) {
-    if (out16) cudaMemcpyFromSymbol(out16, linmin::g_phase, 16 * sizeof(unsigned long long));
-    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(linmin::g_phase, z, sizeof(z)); }
-    return 0;
-}
-#endif
-
 int linmin_version(void) { return LINMIN_VERSION; }
 
 int linmin_trim_memory(void) {
     std::lock_guard<std::mutex> lk(g_pool_mu);
     for (cudaMemPool_t pool : g_pools)
         if (pool && cudaMemPoolTrimTo(pool, 0) != cudaSuccess) { (void)cudaGetLastError(); return LINMIN_ERR_CUDA; }
-    return LINMIN_OK;
-}
-
-int linmin_probe_fp32_peak(void *stream, double *ffma_tflops, double *ffma2_tflops) {
-    if (!ffma_tflops || !ffma2_tflops) return LINMIN_ERR_INVALID_ARGUMENT;
-    int dev = 0, sms = 0;
-    CK(cudaGetDevice(&dev));
-    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CK(probe_fp32(sms, (cudaStream_t)stream, ffma_tflops, ffma2_tflops));
     return LINMIN_OK;
 }
 
@@ -391,38 +363,41 @@ int linmin_library_create(const float *A, int32_t L, int32_t R, const linmin_opt
         if (opts->struct_size != sizeof(linmin_opts)) return LINMIN_ERR_INVALID_ARGUMENT;
         stream = (cudaStream_t)opts->stream;
     }
-    return library_create_impl(A, L, R, stream, false, lib);
+    return library_create_impl(A, L, R, stream, false, true, lib);
 }
 
 void linmin_library_destroy(linmin_library *lib) {
     if (!lib) return;
     cudaStream_t s = lib->stream;
-    if (lib->A) cudaFreeAsync(lib->A, s);
-    if (lib->At) cudaFreeAsync(lib->At, s);
-    if (lib->Ac) cudaFreeAsync(lib->Ac, s);
-    if (lib->c) cudaFreeAsync(lib->c, s);
-    if (lib->Gc) cudaFreeAsync(lib->Gc, s);
-    if (lib->Gi) cudaFreeAsync(lib->Gi, s);
-    if (lib->Giq) cudaFreeAsync(lib->Giq, s);
-    if (lib->G64) cudaFreeAsync(lib->G64, s);
+    {   // the frees below are ordered on the creation stream: make it wait for the last work of every other stream
+        std::lock_guard<std::mutex> lk(lib->use_mu);
+        if (lib->use_overflow) cudaDeviceSynchronize();
+        for (int i = 0; i < lib->n_use; ++i) {
+            cudaStreamWaitEvent(s, lib->use_event[i], 0);
+            cudaEventDestroy(lib->use_event[i]);
+        }
+        lib->n_use = 0;
+    }
+    void *bufs[] = {lib->A, lib->At, lib->Ac, lib->c, lib->Gc, lib->Gi, lib->Giq, lib->scal, lib->G64, lib->W64, lib->flags};
+    for (void *q : bufs) if (q) cudaFreeAsync(q, s);
     for (int i = 0; i < 3; ++i) if (lib->ev[i]) cudaEventDestroy(lib->ev[i]);
     (void)cudaGetLastError();
     delete lib;
 }
 
-int linmin_library_last_launches(const linmin_library *lib) { return lib ? lib->last_launches : 0; }
+int linmin_library_last_launches(const linmin_library *lib) { return lib ? lib->last_launches.load() : 0; }
 
 int linmin_library_enable_timing(linmin_library *lib, int enable) {
     if (!lib) return LINMIN_ERR_INVALID_ARGUMENT;
     if (enable && !lib->ev[0])
         for (int i = 0; i < 3; ++i) CK(cudaEventCreate(&lib->ev[i]));
     lib->timing = enable != 0;
-    lib->timed = false;
+    lib->timed.store(false);
     return LINMIN_OK;
 }
 
 int linmin_library_last_timing(const linmin_library *lib, float *ipls_ms, float *finish_ms) {
-    if (!lib || !lib->timing || !lib->timed) return LINMIN_ERR_INVALID_ARGUMENT;
+    if (!lib || !lib->timing || !lib->timed.load()) return LINMIN_ERR_INVALID_ARGUMENT;
     CK(cudaEventSynchronize(lib->ev[2]));
     float a = 0.0f, b = 0.0f;
     CK(cudaEventElapsedTime(&a, lib->ev[0], lib->ev[1]));
@@ -439,8 +414,12 @@ int linmin_unmix_lib(const linmin_library *lib, const float *Y, const float *sig
     Resolved o;
     int rc = resolve_opts(opts, lib->L, &o);
     if (rc != LINMIN_OK) return rc;
-    if (N == 0) { lib->last_launches = 0; return LINMIN_OK; }
+    if (N >= ((int64_t)1 << 32)) return LINMIN_ERR_UNSUPPORTED_SIZE;
+    if (N == 0) { lib->last_launches.store(0); return LINMIN_OK; }
     if (!Y || !coeffs_out) return LINMIN_ERR_INVALID_ARGUMENT;
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev != lib->device) return LINMIN_ERR_INVALID_ARGUMENT;     // the handle's memory lives on another device
     return launch_solve(lib, Y, sigma, N, o, coeffs_out, coeff_sigma_out, resid_out);
 }
 
@@ -454,10 +433,20 @@ int linmin_unmix(const float *A, const float *Y, const float *sigma, int64_t N, 
     if (rc != LINMIN_OK) return rc;
     if (N > 0 && (!Y || !coeffs_out)) return LINMIN_ERR_INVALID_ARGUMENT;
     linmin_library *lib = nullptr;
-    int wrc = library_create_impl(A, L, R, o.stream, false, &lib);
+    // everything is enqueued on the caller's stream and the call returns: no synchronisation, no host arithmetic.
+    // A non-finite library can therefore not be reported through the status: the solve kernels return at once on
+    // the device flag and the outputs are poisoned instead (NaN, LINMIN_INFO_LIBRARY_NONFINITE).
+    int wrc = library_create_impl(A, L, R, o.stream, false, false, &lib);
     if (wrc < 0) return wrc;
     rc = LINMIN_OK;
-    if (N > 0) rc = launch_solve(lib, Y, sigma, N, o, coeffs_out, coeff_sigma_out, resid_out);
+    if (N > 0) {
+        rc = launch_solve(lib, Y, sigma, N, o, coeffs_out, coeff_sigma_out, resid_out);
+        if (rc == LINMIN_OK) {
+            const int grid = (int)std::min<int64_t>((N * R + 255) / 256, (int64_t)lib->sm_count * 8);
+            poison_outputs_kernel<<<grid, 256, 0, o.stream>>>(lib->flags, N, R, coeffs_out, coeff_sigma_out, resid_out, o.info);
+            if (cudaGetLastError() != cudaSuccess) rc = LINMIN_ERR_CUDA;
+        }
+    }
     linmin_library_destroy(lib);   // stream-ordered frees: safe while the kernels are still queued
     return rc != LINMIN_OK ? rc : wrc;
 }
@@ -499,7 +488,7 @@ int linmin_unmix_host(const float *A, const float *Y, const float *sigma, int64_
         cudaError_t e__ = (call);                                                   \
         if (e__ != cudaSuccess) { (void)cudaGetLastError(); cleanup(); return cuda_status(e__); } \
     } while (0)
-    wrc = library_create_impl(A, L, R, nullptr, true, &lib);
+    wrc = library_create_impl(A, L, R, nullptr, true, true, &lib);
     if (wrc < 0) { lib = nullptr; return wrc; }
     if (N == 0) { cleanup(); return wrc; }
     const bool per_pixel_sigma = sigma && o.sstride != 0;

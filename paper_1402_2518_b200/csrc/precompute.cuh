@@ -57,4 +57,84 @@ __global__ void gram_kernel(const float *__restrict__ A, const float *__restrict
     Gc[e] = (float)sc;
 }
 
+// Start-point data of IPLS (the "factor data" of north_star's precompute step): Gi = (Gc + 1e-4 gdmax I)^-1, its
+// row sums Giq, and gdmax = max_i Gc[i][i] -- on the device, so that the library precompute has no host round
+// trip.  ONE CTA; W is an R x R fp64 workspace in global memory (512 KB at R = 256: more than shared memory
+// holds).  The regularised matrix is symmetric positive definite with a condition number <= 1e4 R, so the in-place
+// Gauss-Jordan inversion needs no pivoting in fp64.  Step j: the pivot row and column go to shared memory, every
+// other entry is updated from them.  scal[0] = gdmax (1 when every G_ii is 0: all endmembers identical, any point
+// of the simplex is optimal), scal[1] = sum of Giq.
+__global__ void __launch_bounds__(1024, 1)
+start_data_kernel(const float *__restrict__ Gc, int R, double *__restrict__ W, float *__restrict__ Gi,
+                  float *__restrict__ Giq, float *__restrict__ scal) {
+    __shared__ double prow[LINMIN_MAX_R], pcol[LINMIN_MAX_R];
+    __shared__ float red[32];
+    const int tid = threadIdx.x, nt = blockDim.x;
+    float gd = 0.0f;
+    for (int i = tid; i < R; i += nt) gd = fmaxf(gd, Gc[(size_t)i * R + i]);
+    gd = warp_max(gd);
+    if ((tid & 31) == 0) red[tid >> 5] = gd;
+    __syncthreads();
+    gd = 0.0f;
+    for (int w = 0; w < (nt >> 5); ++w) gd = fmaxf(gd, red[w]);
+    if (!(gd > 0.0f)) gd = 1.0f;
+    const double delta = 1e-4 * (double)gd;
+    for (int e = tid; e < R * R; e += nt) {
+        const int i = e / R, j = e - i * R;
+        // symmetrised read: Gc is symmetric up to the order of its fp64 sums
+        W[e] = 0.5 * ((double)Gc[e] + (double)Gc[(size_t)j * R + i]) + (i == j ? delta : 0.0);
+    }
+    __syncthreads();
+    for (int j = 0; j < R; ++j) {
+        for (int i = tid; i < R; i += nt) { prow[i] = W[(size_t)j * R + i]; pcol[i] = W[(size_t)i * R + j]; }
+        __syncthreads();
+        const double d = prow[j];
+        const double pv = 1.0 / ((d > 0.0) ? d : delta);
+        for (int e = tid; e < R * R; e += nt) {
+            const int i = e / R, c = e - i * R;
+            double v;
+            if (i == j) v = (c == j) ? pv : prow[c] * pv;
+            else if (c == j) v = -pcol[i] * pv;
+            else v = W[e] - pcol[i] * pv * prow[c];
+            W[e] = v;
+        }
+        __syncthreads();
+    }
+    // symmetrise, round once to fp32, row sums in fp64
+    for (int i = tid; i < R; i += nt) {
+        double q = 0.0;
+        for (int j = 0; j < R; ++j) {
+            const double v = 0.5 * (W[(size_t)i * R + j] + W[(size_t)j * R + i]);
+            Gi[(size_t)i * R + j] = (float)v;
+            q += v;
+        }
+        Giq[i] = (float)q;
+        prow[i] = (double)(float)q;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double s = 0.0;
+        for (int i = 0; i < R; ++i) s += prow[i];
+        scal[0] = gd;
+        scal[1] = (float)s;
+    }
+}
+
+// One-shot calls do not wait for the library check: when the library turned out non-finite, every output of the
+// call is overwritten with NaN and every info word with LINMIN_INFO_LIBRARY_NONFINITE (include/linmin.h).
+__global__ void poison_outputs_kernel(const int *__restrict__ flags, int64_t N, int R, float *__restrict__ coeffs,
+                                      float *__restrict__ csig, float *__restrict__ resid, int32_t *__restrict__ info) {
+    if (!(flags[0] & 1)) return;
+    const float qnan = __int_as_float(0x7fc00000);
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < N * R; e += stride) {
+        coeffs[e] = qnan;
+        if (csig) csig[e] = qnan;
+    }
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < N; p += stride) {
+        if (resid) resid[p] = qnan;
+        if (info) info[p] = LINMIN_INFO_LIBRARY_NONFINITE;
+    }
+}
+
 }  // namespace linmin

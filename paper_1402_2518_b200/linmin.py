@@ -29,10 +29,11 @@ INFO_NONFINITE_INPUT = 0x04
 INFO_CHOL_REGULARISED = 0x08
 INFO_FINISH_FALLBACK = 0x10
 INFO_BAD_SIGMA = 0x20
+INFO_LIBRARY_NONFINITE = 0x40
 
 EXPORTS = ["linmin_version", "linmin_strerror", "linmin_library_create", "linmin_library_destroy",
            "linmin_library_last_launches", "linmin_library_enable_timing", "linmin_library_last_timing",
-           "linmin_probe_fp32_peak", "linmin_trim_memory",
+           "linmin_trim_memory",
            "linmin_unmix_lib", "linmin_unmix", "linmin_unmix_host"]
 
 
@@ -72,7 +73,6 @@ def load() -> ctypes.CDLL:
         lib.linmin_library_last_launches.argtypes = [P]
         lib.linmin_library_enable_timing.argtypes = [P, ctypes.c_int]
         lib.linmin_library_last_timing.argtypes = [P, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]
-        lib.linmin_probe_fp32_peak.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
         lib.linmin_unmix_lib.argtypes = [P, P, P, I64, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_unmix.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_unmix_host.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
@@ -185,19 +185,46 @@ def trim_memory() -> None:
     _check(load().linmin_trim_memory())
 
 
-def probe_fp32_peak(stream=None):
-    """(FFMA TFLOP/s, FFMA2 TFLOP/s) sustained by the FMA pipe of the current device (report helper)."""
-    a, b = ctypes.c_double(), ctypes.c_double()
-    _check(load().linmin_probe_fp32_peak(None if stream is None else ctypes.c_void_p(stream), ctypes.byref(a), ctypes.byref(b)))
-    return a.value, b.value
-
-
 def library_create(A) -> Library:
     return Library(A)
 
 
 def library_destroy(lib: Library) -> None:
     lib.destroy()
+
+
+def _check_tensor(t, name, shape, dtype, cuda, device=None):
+    """Argument marshalling guard: the C ABI reads and writes exactly shape x dtype through data_ptr()."""
+    if t is None:
+        return
+    if tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name} must have shape {tuple(shape)}, got {tuple(t.shape)}")
+    if t.dtype != dtype:
+        raise ValueError(f"{name} must be {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    if bool(t.is_cuda) != bool(cuda):
+        raise ValueError(f"{name} must be a {'CUDA' if cuda else 'CPU'} tensor")
+    if cuda and device is not None and t.device != device:
+        raise ValueError(f"{name} must live on {device}")
+
+
+def _check_outputs(N, R, coeffs, csig, resid, info, cuda, device=None):
+    torch = _torch()
+    _check_tensor(coeffs, "out['coeffs']", (N, R), torch.float32, cuda, device)
+    _check_tensor(csig, "out['coeff_sigma']", (N, R), torch.float32, cuda, device)
+    _check_tensor(resid, "out['resid']", (N,), torch.float32, cuda, device)
+    _check_tensor(info, "out['info']", (N,), torch.int32, cuda, device)
+
+
+def _check_sigma(sigma, N, L, cuda, device=None):
+    torch = _torch()
+    if sigma is None:
+        return
+    if sigma.dim() == 1:
+        _check_tensor(sigma, "sigma", (L,), torch.float32, cuda, device)
+    else:
+        _check_tensor(sigma, "sigma", (N, L), torch.float32, cuda, device)
 
 
 def _alloc_outputs(N, R, device, want_sigma, want_resid, want_info, out):
@@ -215,6 +242,7 @@ def _alloc_outputs(N, R, device, want_sigma, want_resid, want_info, out):
     info = out.get("info")
     if info is None and want_info:
         info = torch.empty((N,), dtype=torch.int32, device=device)
+    _check_outputs(N, R, coeffs, csig, resid, info, True, device)
     return coeffs, csig, resid, info
 
 
@@ -230,6 +258,11 @@ def unmix_lib(lib: Library, Y, sigma=None, *, want_sigma=True, want_resid=True, 
     ldY = int(Y.stride(0)) if N > 1 else lib.L
     if Y.stride(1) != 1 and N > 0:
         raise ValueError("spectra must be contiguous along channels")
+    if not Y.is_cuda or Y.dtype != torch.float32:
+        raise ValueError("Y must be a CUDA float32 tensor")
+    if Y.device != lib.device:
+        raise ValueError(f"Y must live on the library's device {lib.device}")
+    _check_sigma(sigma, N, lib.L, True, Y.device)
     coeffs, csig, resid, info = _alloc_outputs(N, lib.R, Y.device, want_sigma, want_resid, want_info, out)
     with torch.cuda.device(Y.device):
         o = _make_opts(stream=torch.cuda.current_stream().cuda_stream, ldY=ldY,
@@ -237,8 +270,6 @@ def unmix_lib(lib: Library, Y, sigma=None, *, want_sigma=True, want_resid=True, 
                        weighting=weighting, max_iter=max_iter, gap_tol=gap_tol, feas_tol=feas_tol,
                        info_ptr=None if info is None else info.data_ptr())
         yp = ctypes.c_void_p(Y.data_ptr()) if N > 0 else None
-        if N > 0 and (not Y.is_cuda or Y.dtype != torch.float32):
-            raise ValueError("Y must be a CUDA float32 tensor")
         st = _check(load().linmin_unmix_lib(lib._h, yp, _dev_ptr(sigma, "sigma"), N, ctypes.byref(o),
                                             _dev_ptr(coeffs, "coeffs"), _dev_ptr(csig, "coeff_sigma"),
                                             _dev_ptr(resid, "resid")))
@@ -249,8 +280,15 @@ def unmix(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=True,
           out: Optional[dict] = None, max_iter=0, gap_tol=0.0, feas_tol=0.0, constraint=0, weighting=0):
     """linmin_unmix (one-shot: precompute + solve).  All tensors CUDA float32."""
     torch = _torch()
+    if A.dim() != 2:
+        raise ValueError("A must be (L, R)")
     L, R = int(A.shape[0]), int(A.shape[1])
+    _check_tensor(A, "A", (L, R), torch.float32, True)
+    if Y.dim() != 2 or int(Y.shape[1]) != L:
+        raise ValueError("Y must be (N, L)")
     N = int(Y.shape[0])
+    _check_tensor(Y, "Y", (N, L), torch.float32, True, A.device)
+    _check_sigma(sigma, N, L, True, A.device)
     coeffs, csig, resid, info = _alloc_outputs(N, R, A.device, want_sigma, want_resid, want_info, out)
     with torch.cuda.device(A.device):
         o = _make_opts(stream=torch.cuda.current_stream().cuda_stream, ldY=0,
@@ -280,8 +318,13 @@ def unmix_host(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=
         return t
 
     A, Y, sigma = as_cpu(A, "A"), as_cpu(Y, "Y"), as_cpu(sigma, "sigma")
+    if A.dim() != 2:
+        raise ValueError("A must be (L, R)")
     L, R = int(A.shape[0]), int(A.shape[1])
+    if Y.dim() != 2 or int(Y.shape[1]) != L:
+        raise ValueError("Y must be (N, L)")
     N = int(Y.shape[0])
+    _check_sigma(sigma, N, L, False)
     out = dict(out or {})
     pin = torch.cuda.is_available()
 
@@ -298,6 +341,7 @@ def unmix_host(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=
     info = out.get("info")
     if info is None and want_info:
         info = host_empty((N,), torch.int32)
+    _check_outputs(N, R, coeffs, csig, resid, info, False)
     o = _make_opts(ldY=0, sigma_pixel_stride=_sigma_stride(sigma, N, L), max_iter=max_iter,
                    gap_tol=gap_tol, feas_tol=feas_tol, info_ptr=None if info is None else info.data_ptr())
 

@@ -6,6 +6,10 @@ Tolerances are north_star's (BASELINE.json), read as in DESIGN.md R10/R12:
   resid within 1e-5 relative (same floor), coeff_sigma within 1 % relative (+1e-7 absolute) where the
   supports agree; where they differ (ties, R10) the GPU value is compared with reading R3 evaluated
   in numpy ON THE GPU's support, and the number of such pixels must stay below 0.5 %.
+
+Before the oracle's answer is used as the reference for a pixel it is itself certified HERE, in numpy,
+independently of oracle/ (check_oracle_kkt): the scaled optimality conditions of the problem (R11) on its
+coefficients, and its multipliers against the recomputed ones, for EVERY compared pixel.
 """
 import numpy as np
 
@@ -25,14 +29,56 @@ def sigma_reference_on_support(A64, F, sig):
     return out
 
 
-def check_parity(A, Y, sigma, gpu, ora, label="", require_unique=True):
-    """gpu: dict(coeffs, coeff_sigma, resid) numpy float32 arrays for the SAME pixels as ora."""
+def check_oracle_kkt(A, Y, ora, label="", tol=1e-9, chunk=65536):
+    """Optimality conditions of eq. 2 under eq. 3-4 for the ORACLE's coefficients, recomputed
+    in numpy from the coefficients alone, on every pixel handed in (scaled as reading R11): sum a = 1, a >= 0,
+    multipliers >= -tol, complementarity and stationarity on the support <= tol, all relative to ||g||_inf plus the
+    rounding scale of g (1e-13 max_i sum_l |A_li||y_l|: g = 0 exactly on a noiseless pixel).  Also compares the
+    oracle's own lambda / nu outputs with the recomputed ones.  A pixel on which the oracle blocked an index
+    (rank loss or degenerate tie) is certified like any other: a wrongly blocked index shows up as a negative
+    multiplier here."""
+    A64 = A.astype(np.float64)
+    absA = np.abs(A64)
+    worst = dict(sum=0.0, neg=0.0, lam_neg=0.0, stat=0.0, lam_out=0.0, nu_out=0.0)
+    N = Y.shape[0]
+    for p0 in range(0, N, chunk):
+        sl = slice(p0, min(N, p0 + chunk))
+        a = ora.coeffs[sl]
+        y = Y[sl].astype(np.float64)
+        ok = np.isfinite(y).all(1)
+        a, y = a[ok], y[ok]
+        if a.shape[0] == 0:
+            continue
+        g = (a @ A64.T - y) @ A64                      # gradient of F/2
+        F = a > 0
+        nu = -(g * a).sum(1)
+        scale = np.abs(g).max(1) + 1e-4 * (np.abs(y) @ absA).max(1)   # 1e-4 * tol = the 1e-13 rounding floor
+        lam = np.where(F, 0.0, g + nu[:, None])
+        worst["sum"] = max(worst["sum"], float(np.abs(a.sum(1) - 1.0).max()))
+        worst["neg"] = max(worst["neg"], float(max(0.0, -a.min())))
+        worst["lam_neg"] = max(worst["lam_neg"], float((np.maximum(0.0, -lam.min(1)) / scale).max()))
+        worst["stat"] = max(worst["stat"], float((np.abs(np.where(F, g + nu[:, None], 0.0)).max(1) / scale).max()))
+        worst["lam_out"] = max(worst["lam_out"], float((np.abs(ora.lam[sl][ok] - lam).max(1) / scale).max()))
+        worst["nu_out"] = max(worst["nu_out"], float((np.abs(ora.nu[sl][ok] - nu) / scale).max()))
+    assert worst["sum"] <= 1e-12, (label, "oracle KKT", worst)
+    assert worst["neg"] == 0.0, (label, "oracle KKT", worst)
+    assert worst["lam_neg"] <= tol, (label, "oracle KKT", worst)
+    assert worst["stat"] <= tol, (label, "oracle KKT", worst)
+    assert worst["lam_out"] <= tol and worst["nu_out"] <= tol, (label, "oracle multipliers", worst)
+    return worst
+
+
+def check_parity(A, Y, sigma, gpu, ora, label="", min_unique=0.99, max_tie_frac=0.005):
+    """gpu: dict(coeffs, coeff_sigma, resid) numpy float32 arrays for the SAME pixels as ora.
+    min_unique: asserted lower bound on the fraction of pixels whose minimiser is unique (R9) and on which the
+    coefficients and uncertainties are therefore compared element by element."""
     A64 = A.astype(np.float64)
     Y64 = Y.astype(np.float64)
     a = gpu["coeffs"].astype(np.float64)
     N, R = a.shape
     L = A.shape[0]
     assert np.isfinite(a).all(), label
+    kkt = check_oracle_kkt(A, Y, ora, label)
     # feasibility
     assert np.abs(a.sum(1) - 1.0).max() <= 1e-5, (label, np.abs(a.sum(1) - 1.0).max())
     assert a.min() >= -1e-6, (label, a.min())
@@ -42,14 +88,16 @@ def check_parity(A, Y, sigma, gpu, ora, label="", require_unique=True):
     floor = 1e-12 * (Y64 ** 2).sum(1)
     rel = np.abs(Fg - Fo) / np.maximum(Fo, floor)
     assert rel.max() <= 1e-5, (label, "objective", rel.max(), int(rel.argmax()))
-    # coefficients: where the minimiser is unique (R9)
+    # coefficients: where the minimiser is unique (R9); the mask is pinned by tests/test_oracle_pins.py::
+    # test_rank_margin_* and its size is asserted, never just printed
     sing = np.linalg.svd(A64, compute_uv=False)
     unique = ora.rank_margin > 1e-6 * sing[0]
-    if require_unique:
-        assert unique.mean() > 0.99, (label, unique.mean())
+    assert unique.mean() >= min_unique, (label, "unique fraction", unique.mean(), min_unique)
+    assert unique.any(), (label, "no pixel with a unique minimiser")
     da = np.abs(a - ora.coeffs).max(1)
     assert da[unique].max() <= 1e-4, (label, "coeffs", da[unique].max(), int(np.argmax(np.where(unique, da, 0))))
-    stats = dict(max_da=float(da[unique].max()), max_rel_obj=float(rel.max()), n_nonunique=int((~unique).sum()))
+    stats = dict(pixels=int(N), max_da=float(da[unique].max()), max_rel_obj=float(rel.max()),
+                 n_nonunique=int((~unique).sum()), oracle_kkt=max(kkt["lam_neg"], kkt["stat"]))
     # residual
     if gpu.get("resid") is not None:
         rg = gpu["resid"].astype(np.float64)
@@ -63,9 +111,10 @@ def check_parity(A, Y, sigma, gpu, ora, label="", require_unique=True):
         Fo_sup = ora.coeffs > 0
         same = (Fg_sup == Fo_sup).all(1)
         err = np.abs(sg - ora.coeff_sigma) - (0.01 * ora.coeff_sigma + 1e-7)
-        assert err[same & unique].max() <= 0, (label, "sigma", err[same & unique].max())
+        if (same & unique).any():
+            assert err[same & unique].max() <= 0, (label, "sigma", err[same & unique].max())
         ties = np.nonzero(~same & unique)[0]
-        assert len(ties) <= max(2, 0.005 * N), (label, "support mismatches", len(ties))
+        assert len(ties) <= max(2, max_tie_frac * N), (label, "support mismatches", len(ties))
         for p in ties:
             # the differing members must be marginal (tiny coefficient on either side)
             diff = Fg_sup[p] ^ Fo_sup[p]

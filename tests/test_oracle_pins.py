@@ -374,3 +374,87 @@ def test_degenerate_cases():
     # empty batch
     r0 = oracle.solve(A, np.zeros((0, L), np.float32))
     assert r0.coeffs.shape == (0, 4)
+
+
+# ---------------------------------------------------------------- rank margin (R9): the uniqueness mask of tests/parity.py
+def _sigma_min_AFZ(A64, F):
+    """sigma_min(A_F Z) from numpy's SVD, Z = ANY orthonormal basis of {z : 1'z = 0} (here from numpy's QR of
+    [1 | I]; the singular values do not depend on the choice)."""
+    k = len(F)
+    Q, _ = np.linalg.qr(np.concatenate([np.ones((k, 1)), np.eye(k)[:, : k - 1]], axis=1))
+    Z = Q[:, 1:]
+    assert np.abs(Z.sum(0)).max() < 1e-12
+    return np.linalg.svd(A64[:, F] @ Z, compute_uv=False)[-1]
+
+
+@pytest.mark.parametrize("name,n", [("tiny", 400), ("omega", 400), ("crism", 150), ("stress", 120)])
+def test_rank_margin_brackets_sigma_min(name, n):
+    """rank_margin (smallest |R_jj| of the column-pivoted QR of A_F Z on the final support) decides which pixels
+    get element-wise coefficient / sigma assertions (tests/parity.py).  For a column-pivoted QR
+    sigma_min <= min |R_jj| <= sqrt(m) 2^(m-1) sigma_min in theory and a small multiple in practice: pin
+    it inside [1, 6] x numpy's sigma_min(A_F Z), so a bookkeeping slip (wrong column, stale value of an earlier
+    support, wrong reduction) cannot silently switch the assertions off."""
+    w = make_workload(name, N=n)
+    res = oracle.solve(w.A, w.Y, w.sigma)
+    A64 = w.A.astype(np.float64)
+    ratios = []
+    for p in range(n):
+        F = np.nonzero(res.coeffs[p] > 0)[0]
+        assert len(F) == res.support_size[p]
+        if len(F) == 1:
+            assert np.isinf(res.rank_margin[p])
+            continue
+        ratios.append(res.rank_margin[p] / _sigma_min_AFZ(A64, F))
+    ratios = np.array(ratios)
+    assert len(ratios) > n // 2
+    assert ratios.min() >= 1.0 - 1e-9 and ratios.max() <= 6.0, (ratios.min(), ratios.max())
+
+
+def test_rank_margin_of_near_duplicate_columns():
+    """Two members that differ by delta: the margin must come out at the size of delta (here ~1e-7 of
+    sigma_max, below the 1e-6 mask of tests/parity.py), and scale with delta."""
+    rng = np.random.default_rng(41)
+    L = 16
+    base = rand_library(rng, L, 3, 0.2).astype(np.float64)
+    v = rng.standard_normal(L)
+    margins = []
+    for delta in (2.0 ** -20, 2.0 ** -17):
+        A = np.concatenate([base, base[:, :1] + delta * v[:, None]], axis=1).astype(np.float32)
+        a0 = np.array([0.3, 0.25, 0.15, 0.3])
+        y = (A.astype(np.float64) @ a0).astype(np.float32)
+        res = oracle.solve(A, y[None])
+        F = np.nonzero(res.coeffs[0] > 0)[0]
+        if len(F) == 4:            # both twins active: the margin is that of the near-dependent pair
+            smin = _sigma_min_AFZ(A.astype(np.float64), F)
+            assert 1.0 - 1e-9 <= res.rank_margin[0] / smin <= 6.0
+            smax = np.linalg.svd(A.astype(np.float64), compute_uv=False)[0]
+            assert res.rank_margin[0] < 1e-5 * smax
+            margins.append(res.rank_margin[0])
+    assert len(margins) == 2 and 6.0 < margins[1] / margins[0] < 10.0      # delta ratio is 8
+    # exact duplicate: the second twin is rejected as rank-deficient and the pixel is flagged
+    Ad = np.concatenate([base, base[:, :1]], axis=1).astype(np.float32)
+    y = (Ad.astype(np.float64) @ np.array([0.3, 0.25, 0.15, 0.3]) + 1e-3 * rng.standard_normal(L)).astype(np.float32)
+    rd = oracle.solve(Ad, y[None])
+    assert rd.coeffs[0, 0] == 0.0 or rd.coeffs[0, 3] == 0.0
+
+
+# ---------------------------------------------------------------- the certificate tests/parity.py runs on every compared pixel
+@pytest.mark.parametrize("name,n", [("tiny", 1000), ("omega", 20000), ("crism", 3000), ("stress", 300)])
+def test_parity_certificate_on_oracle_outputs(name, n):
+    """tests/parity.py::check_oracle_kkt (numpy, independent of oracle/) accepts the oracle's answers, multipliers
+    included, on every pixel; and it rejects a perturbed answer (so it is not vacuous)."""
+    import sys
+    sys.path.insert(0, HERE)
+    from parity import check_oracle_kkt
+    w = make_workload(name, N=n)
+    res = oracle.solve(w.A, w.Y, w.sigma)
+    worst = check_oracle_kkt(w.A, w.Y, res, label=name)
+    assert worst["lam_neg"] <= 1e-9
+    # move 1e-6 of mass between two active members of one pixel, or drop a weakly active member: must be caught
+    p = int(np.argmax(res.support_size))
+    F = np.nonzero(res.coeffs[p] > 0)[0]
+    bad = oracle.OracleResult(*[np.array(getattr(res, f), copy=True) for f in
+                                ("coeffs", "coeff_sigma", "resid", "lam", "nu", "support_size", "steps", "rank_margin", "status")])
+    bad.coeffs[p, F[0]] += 1e-6; bad.coeffs[p, F[1]] -= 1e-6
+    with pytest.raises(AssertionError):
+        check_oracle_kkt(w.A, w.Y, bad, label="perturbed")
