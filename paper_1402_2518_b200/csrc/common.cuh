@@ -24,7 +24,7 @@ struct LibView {
     const float *Ac;    // L x R, centred: Ac[l][r] = A[l][r] - c[l], c[l] = mean_r A[l][r]
     const float *c;     // L
     const float *Gc;    // R x R fp32, Gc = Ac' Ac accumulated in fp64 (drives IPLS)
-    const double *G64;  // R x R fp64, G = A' A (uncentred, exact data; drives the finish)
+    const double *G64;  // R x R fp64, A'A + t 11' (uncentred, exact data; t: precompute.cuh; drives the finish)
     const float *scal;  // device scalars of the precompute: [0] gdmax = max_i Gc[i][i] (1 if that is 0), [1] sum of Giq
     const int *flags;   // device word: bit 0 = the library holds a non-finite value (every kernel then returns at once)
     const float *Gi;    // R x R fp32, (Gc + 1e-4 gdmax I)^-1 (start point of IPLS: regularised sum-constrained LS)

@@ -16,7 +16,7 @@
 #include "finish.cuh"
 #include "finish_fast.cuh"
 #include "ipls_generic.cuh"
-#include "ipls_r32.cuh"
+#include "ipls_q32.cuh"
 #include "precompute.cuh"
 
 using namespace linmin;
@@ -213,9 +213,24 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     CK(cudaMemsetAsync(ws, 0, std::min<size_t>(9, ws_words) * sizeof(unsigned int), o.stream));
     unsigned int *counters = ws, *overflow = ws + 8, *repair = ws + 8 + ((size_t)N + 1);
     if (use_f8) CK(cudaMemsetAsync(repair, 0, sizeof(unsigned int), o.stream));
-    if (R == 32 && ipls_r32_supported(L)) {
-        CK(launch_ipls_r32(lv, prm, lib->sm_count, counters, o.stream));
-        ++launches;
+    if (R == 32 && start_r32_warps(L) > 0) {
+        // K0 (projection + start point, one record per pixel) and K1 (the iteration), in chunks of 2^21 pixels
+        // so that the record workspace stays at 0.8 GB whatever N is
+        const int64_t chunk = (int64_t)1 << 21;
+        const int nchunks = (int)((N + chunk - 1) / chunk);
+        float *recbuf = nullptr;
+        unsigned int *tickets = nullptr;
+        CK(staging_alloc((void **)&recbuf, (size_t)std::min(N, chunk) * s32::REC * sizeof(float), o.stream));
+        struct FreeF { void *p; cudaStream_t s; ~FreeF() { cudaFreeAsync(p, s); } } free_rec{recbuf, o.stream};
+        CK(staging_alloc((void **)&tickets, (size_t)nchunks * sizeof(unsigned int), o.stream));
+        FreeF free_tk{tickets, o.stream};
+        CK(cudaMemsetAsync(tickets, 0, (size_t)nchunks * sizeof(unsigned int), o.stream));
+        for (int c = 0; c < nchunks; ++c) {
+            const int64_t pb = (int64_t)c * chunk, pe = std::min(N, pb + chunk);
+            CK(launch_start_r32(lv, prm, pb, pe, recbuf, lib->sm_count, o.stream));
+            CK(launch_ipls_q32(lv, prm, pb, pe, recbuf, lib->sm_count, tickets + c, o.stream));
+            launches += 2;
+        }
     } else if (R <= 64) {
         const int teams = 8, block = teams * 32;
         size_t smem = teams * ipls_warp_team_floats(L, R) * sizeof(float);
@@ -311,7 +326,7 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
         gram_kernel<<<grid, block, 0, stream>>>(lib->A, lib->Ac, L, R, lib->G64, lib->Gc);
         CKF(cudaGetLastError());
         // start point data of IPLS: inverse of the regularised centred Gram matrix, its row sums, gdmax
-        start_data_kernel<<<1, 1024, 0, stream>>>(lib->Gc, R, lib->W64, lib->Gi, lib->Giq, lib->scal);
+        start_data_kernel<<<1, 1024, 0, stream>>>(lib->Gc, R, lib->W64, lib->Gi, lib->Giq, lib->scal, lib->G64, 1);
         CKF(cudaGetLastError());
     }
     if (wait_check) {

@@ -63,10 +63,17 @@ __global__ void gram_kernel(const float *__restrict__ A, const float *__restrict
 // holds).  The regularised matrix is symmetric positive definite with a condition number <= 1e4 R, so the in-place
 // Gauss-Jordan inversion needs no pivoting in fp64.  Step j: the pivot row and column go to shared memory, every
 // other entry is updated from them.  scal[0] = gdmax (1 when every G_ii is 0: all endmembers identical, any point
-// of the simplex is optimal), scal[1] = sum of Giq.
+// of the simplex is optimal), scal[1] = sum of Giq, scal[2] = t (below).
+//
+// The finish solves its equality-constrained sub-problems through the fp64 Gram block of the support.  A_F'A_F is
+// singular as soon as the members are LINEARLY dependent (an all-zero "dark" endmember, or the slack column of the
+// sum-lower-than-one option), although the sub-problem only needs them AFFINELY independent.  Because 1'a = 1
+// (eq. 4), a'(G + t 11')a = a'Ga + t on the feasible set: with G64 <- A'A + t 11', t = max_i G_ii, the
+// minimiser, the multipliers (taken from the data-space residual) and the projected inverse H = K - K11'K/(1'K1)
+// are unchanged, and the block is non-singular exactly when the sub-problem is well posed.  `shift` = 0 skips it.
 __global__ void __launch_bounds__(1024, 1)
 start_data_kernel(const float *__restrict__ Gc, int R, double *__restrict__ W, float *__restrict__ Gi,
-                  float *__restrict__ Giq, float *__restrict__ scal) {
+                  float *__restrict__ Giq, float *__restrict__ scal, double *__restrict__ G64, int shift) {
     __shared__ double prow[LINMIN_MAX_R], pcol[LINMIN_MAX_R];
     __shared__ float red[32];
     const int tid = threadIdx.x, nt = blockDim.x;
@@ -118,6 +125,16 @@ start_data_kernel(const float *__restrict__ Gc, int R, double *__restrict__ W, f
         scal[0] = gd;
         scal[1] = (float)s;
     }
+    // ---- G64 <- A'A + t 11'
+    __syncthreads();
+    for (int i = tid; i < R; i += nt) pcol[i] = G64[(size_t)i * R + i];
+    __syncthreads();
+    double tsh = 0.0;
+    for (int i = 0; i < R; ++i) tsh = fmax(tsh, pcol[i]);
+    if (!shift) tsh = 0.0;
+    __syncthreads();
+    for (int e = tid; e < R * R; e += nt) G64[e] += tsh;
+    if (tid == 0) scal[2] = (float)tsh;
 }
 
 // One-shot calls do not wait for the library check: when the library turned out non-finite, every output of the
