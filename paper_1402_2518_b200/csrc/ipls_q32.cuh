@@ -33,7 +33,8 @@ constexpr int S = 8;            // rows per lane
 constexpr int WARPS = 8;        // warps per CTA, one CTA per SM (255 registers)
 constexpr int GST = 36;         // padded row stride of G in shared memory (conflict-free LDS.128 over the 4 lanes)
 constexpr int XST = 36;         // one exchange line: 32 column entries + pad
-constexpr int PIXF = 100;       // floats per pixel: two exchange lines; 100 = 4 mod 32 spreads the 8 pixels of a warp
+constexpr int PRK = 72;         // offset of the park area: a, lambda, G a - b wait here during the factorisation ([3][4 lanes][8])
+constexpr int PIXF = 196;       // floats per pixel: two exchange lines + park area; 196 = 4 mod 32 spreads the 8 pixels of a warp
 constexpr int QD = 8;           // prefetch queue depth (records) per warp
 constexpr int REC = s32::REC;
 constexpr int BLK = 256;        // pixels a warp reserves per ticket
@@ -52,10 +53,12 @@ __host__ __device__ inline size_t smem_floats() {
 
 // L' x = y in place.  m2 holds -L (strictly lower), ct[s][0..2] the lane's column of the inverse of diagonal block s
 // (coefficients of the block's totals 1..3; the coefficient of total 0 is [t == 0]).
-__device__ __forceinline__ void backward_subst(const float2 (&m2)[S][2 * S], const float (&ct)[S][3], float (&y)[S], int t) {
+__device__ __forceinline__ void backward_subst(const float2 (&m2)[S][2 * S], const float (&ct)[S][3], float (&y)[S], int t,
+                                               const float2 e2a, const float2 e2b) {
 #pragma unroll
     for (int s = S - 1; s >= 0; --s) {
-        float2 pa = make_float2(0.0f, 0.0f), pb = make_float2(0.0f, 0.0f);
+        // my own right-hand side enters at my position of the block (one-hot pairs), then the later rows' shares
+        float2 pa = make_float2(y[s] * e2a.x, y[s] * e2a.y), pb = make_float2(y[s] * e2b.x, y[s] * e2b.y);
         float2 qa = make_float2(0.0f, 0.0f), qb = make_float2(0.0f, 0.0f);
 #pragma unroll
         for (int sp = s + 1; sp < S; ++sp) {
@@ -63,13 +66,11 @@ __device__ __forceinline__ void backward_subst(const float2 (&m2)[S][2 * S], con
             else { qa = fma2(y[sp], m2[sp][2 * s], qa); qb = fma2(y[sp], m2[sp][2 * s + 1], qb); }
         }
         float v0 = pa.x + qa.x, v1 = pa.y + qa.y, v2 = pb.x + qb.x, v3 = pb.y + qb.y;
-        v0 += (t == 0) ? y[s] : 0.0f; v1 += (t == 1) ? y[s] : 0.0f;
-        v2 += (t == 2) ? y[s] : 0.0f; v3 += (t == 3) ? y[s] : 0.0f;
         v0 += __shfl_xor_sync(FULL, v0, 1); v1 += __shfl_xor_sync(FULL, v1, 1);
         v2 += __shfl_xor_sync(FULL, v2, 1); v3 += __shfl_xor_sync(FULL, v3, 1);
         v0 += __shfl_xor_sync(FULL, v0, 2); v1 += __shfl_xor_sync(FULL, v1, 2);
         v2 += __shfl_xor_sync(FULL, v2, 2); v3 += __shfl_xor_sync(FULL, v3, 2);
-        float x = (t == 0) ? v0 : 0.0f;
+        float x = e2a.x * v0;
         x = fmaf(ct[s][0], v1, x);
         x = fmaf(ct[s][1], v2, x);
         x = fmaf(ct[s][2], v3, x);
@@ -238,6 +239,16 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
             m2[s][2 * s + 1] = fma2(d, e2b, m2[s][2 * s + 1]);
             rr[s] = make_float2(1.0f, -(gmb[s] + nu));
         }
+        // the pixel's vectors wait in shared memory while the factorisation needs every register
+        {
+            float *pk = xb0 + PRK + 8 * t;
+            *reinterpret_cast<float4 *>(pk) = make_float4(a[0], a[1], a[2], a[3]);
+            *reinterpret_cast<float4 *>(pk + 4) = make_float4(a[4], a[5], a[6], a[7]);
+            *reinterpret_cast<float4 *>(pk + 32) = make_float4(lam[0], lam[1], lam[2], lam[3]);
+            *reinterpret_cast<float4 *>(pk + 36) = make_float4(lam[4], lam[5], lam[6], lam[7]);
+            *reinterpret_cast<float4 *>(pk + 64) = make_float4(gmb[0], gmb[1], gmb[2], gmb[3]);
+            *reinterpret_cast<float4 *>(pk + 68) = make_float4(gmb[4], gmb[5], gmb[6], gmb[7]);
+        }
         // ---- M = L D L' (right-looking).  m2 ends as -L (strictly lower; zeros on and above the diagonal inside the
         //      diagonal blocks), dinv = 1 / d, ct = my column of the inverse of each diagonal block of L.
         float ct[S][3];
@@ -281,9 +292,10 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
                 const float i20 = fmaf(l21, l10, -l20);
                 const float i31 = fmaf(l32, l21, -l31);
                 const float i30 = fmaf(-l32, i20, fmaf(l31, l10, -l30));
-                ct[s0][0] = (t == 0) ? -l10 : ((t == 1) ? 1.0f : 0.0f);
-                ct[s0][1] = (t == 0) ? i20 : ((t == 1) ? -l21 : ((t == 2) ? 1.0f : 0.0f));
-                ct[s0][2] = (t == 0) ? i30 : ((t == 1) ? i31 : ((t == 2) ? -l32 : 1.0f));
+                // lane t takes column t of the inverse: blended with the one-hot values of t (no divergent branch)
+                ct[s0][0] = fmaf(e2a.x, -l10, e2a.y);
+                ct[s0][1] = fmaf(e2a.x, i20, fmaf(e2a.y, -l21, e2b.x));
+                ct[s0][2] = fmaf(e2a.x, i30, fmaf(e2a.y, i31, fmaf(e2b.x, -l32, e2b.y)));
             }
             // ---- look-ahead: column k + 1 first, then its exchange
             {
@@ -330,6 +342,15 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
             dinv[S - 1] = (t == 3) ? rcp_approx(piv) : dinv[S - 1];
         }
         if (__any_sync(0xfu << (4 * g), clamped)) flags |= LINMIN_INFO_CHOL_REGULARISED;
+        {
+            const float *pk = xb0 + PRK + 8 * t;
+            const float4 a0 = *reinterpret_cast<const float4 *>(pk), a1 = *reinterpret_cast<const float4 *>(pk + 4);
+            const float4 l0 = *reinterpret_cast<const float4 *>(pk + 32), l1 = *reinterpret_cast<const float4 *>(pk + 36);
+            const float4 g0 = *reinterpret_cast<const float4 *>(pk + 64), g1 = *reinterpret_cast<const float4 *>(pk + 68);
+            a[0] = a0.x; a[1] = a0.y; a[2] = a0.z; a[3] = a0.w; a[4] = a1.x; a[5] = a1.y; a[6] = a1.z; a[7] = a1.w;
+            lam[0] = l0.x; lam[1] = l0.y; lam[2] = l0.z; lam[3] = l0.w; lam[4] = l1.x; lam[5] = l1.y; lam[6] = l1.z; lam[7] = l1.w;
+            gmb[0] = g0.x; gmb[1] = g0.y; gmb[2] = g0.z; gmb[3] = g0.w; gmb[4] = g1.x; gmb[5] = g1.y; gmb[6] = g1.z; gmb[7] = g1.w;
+        }
 
         // ---- predictor: M^-1 = L^-T D^-1 L^-1; nu eliminated through L^-1 1
         float sww = 0.0f, swz = 0.0f;
@@ -340,12 +361,12 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
             swz = fmaf(zd, rr[s].y, swz);
         }
         sww = gsum(sww); swz = gsum(swz);
-        const float rsww = 1.0f / sww;
+        const float rsww = rcp_approx(sww);
         float dnu = (swz + rp) * rsww;
         float da[S];
 #pragma unroll
         for (int s = 0; s < S; ++s) da[s] = fmaf(-rr[s].x, dnu, rr[s].y) * dinv[s];
-        backward_subst(m2, ct, da, t);
+        backward_subst(m2, ct, da, t, e2a, e2b);
         float ainv[S];
         float mp = 0.0f, md = 0.0f;     // max of -da/a and -dl/lambda
 #pragma unroll
@@ -364,7 +385,7 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
             mua = fmaf(fmaf(ap, da[s], a[s]), fmaf(ad, dl, lam[s]), mua);
         }
         mua = gsum(mua) * (1.0f / 32.0f);
-        float sg = mua / mu;
+        float sg = mua * rcp_approx(mu);
         sg = fminf(1.0f, fmaxf(0.0f, sg * sg * sg));
         // ---- corrector
         float cc[S], r1[S];
@@ -388,7 +409,7 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
         dnu = (swz + rp) * rsww;
 #pragma unroll
         for (int s = 0; s < S; ++s) da[s] = fmaf(-rr[s].x, dnu, r1[s]) * dinv[s];
-        backward_subst(m2, ct, da, t);
+        backward_subst(m2, ct, da, t, e2a, e2b);
         mp = 0.0f; md = 0.0f;
         float dl[S];
 #pragma unroll
