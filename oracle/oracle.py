@@ -37,6 +37,10 @@ def _load():
         f.argtypes = [P, P, P, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.c_int64,
                       ctypes.c_int64, P, P, P, P, P, P, P, P, P, ctypes.c_int32]
         f.restype = ctypes.c_int
+        fx = lib.linmin_oracle_solve_ex
+        fx.argtypes = [P, P, P, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.c_int64,
+                       ctypes.c_int64, ctypes.c_int32, P, ctypes.c_int32, P, P, P, P, P, P, P, P, P, ctypes.c_int32]
+        fx.restype = ctypes.c_int
         lib.linmin_oracle_max_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -63,9 +67,15 @@ def _ptr(a: Optional[np.ndarray]):
     return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
 
 
+CONSTRAINTS = {"sto": 0, "slo": 1, "pos": 2}
+
+
 def solve(A: np.ndarray, Y: np.ndarray, sigma: Optional[np.ndarray] = None,
-          nthreads: int = 0) -> OracleResult:
-    """A (L,R) float32, Y (N,L) float32, sigma None | (L,) | (N,L) float32."""
+          nthreads: int = 0, constraint: str = "sto", cov: Optional[np.ndarray] = None) -> OracleResult:
+    """A (L,R) float32, Y (N,L) float32, sigma None | (L,) | (N,L) float32.
+    constraint: "sto" (eq. 3 + 4), "slo" (sum lower than one), "pos" (eq. 3 only) -- PAPER.md:35, 157, 221.
+    cov: None (unweighted fit, eq. 2), (L,) per-channel noise std of a diagonal covariance, or (L,L) covariance
+    matrix: the renormalised problem of PAPER.md:77-86 (eq. 5-6); sigma is then ignored."""
     A = np.ascontiguousarray(A, dtype=np.float32)
     Y = np.ascontiguousarray(Y, dtype=np.float32)
     L, R = A.shape
@@ -82,11 +92,23 @@ def solve(A: np.ndarray, Y: np.ndarray, sigma: Optional[np.ndarray] = None,
     out = OracleResult(np.empty((N, R)), np.empty((N, R)), np.empty(N), np.empty((N, R)),
                        np.empty(N), np.empty(N, np.int32), np.empty(N, np.int32), np.empty(N),
                        np.empty(N, np.int32))
-    rc = _load().linmin_oracle_solve(_ptr(A), _ptr(Y), _ptr(sigma), N, L, R, L, stride,
-                                     _ptr(out.coeffs), _ptr(out.coeff_sigma), _ptr(out.resid),
-                                     _ptr(out.lam), _ptr(out.nu), _ptr(out.support_size),
-                                     _ptr(out.steps), _ptr(out.rank_margin), _ptr(out.status),
-                                     int(nthreads))
+    cov_kind = 0
+    if cov is not None:
+        cov = np.ascontiguousarray(cov, dtype=np.float32)
+        if cov.ndim == 1:
+            assert cov.shape == (L,)
+            cov_kind = 1
+        else:
+            assert cov.shape == (L, L)
+            cov_kind = 2
+    rc = _load().linmin_oracle_solve_ex(_ptr(A), _ptr(Y), _ptr(sigma), N, L, R, L, stride,
+                                        CONSTRAINTS[constraint], _ptr(cov), cov_kind,
+                                        _ptr(out.coeffs), _ptr(out.coeff_sigma), _ptr(out.resid),
+                                        _ptr(out.lam), _ptr(out.nu), _ptr(out.support_size),
+                                        _ptr(out.steps), _ptr(out.rank_margin), _ptr(out.status),
+                                        int(nthreads))
+    if rc == -2:
+        raise ValueError("covariance is not positive definite")
     if rc != 0:
         raise RuntimeError(f"linmin_oracle_solve failed with code {rc}")
     if (out.status & 2).any():
