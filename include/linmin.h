@@ -66,23 +66,31 @@ extern "C" {
 #define LINMIN_OK 0
 #define LINMIN_ERR_INVALID_ARGUMENT (-1)  /* NULL required pointer, N < 0, L < 1, R < 1, ldY < L, bad stride, struct_size */
 #define LINMIN_ERR_UNSUPPORTED_SIZE (-2)  /* R > LINMIN_MAX_R or L > LINMIN_MAX_L */
-#define LINMIN_ERR_NOT_IMPLEMENTED (-3)   /* a constraint / weighting option that is not built yet */
+#define LINMIN_ERR_NOT_IMPLEMENTED (-3)   /* kept for ABI stability: every option of this header is implemented */
 #define LINMIN_ERR_CUDA (-4)              /* CUDA runtime failure (including: no device) */
 #define LINMIN_ERR_OUT_OF_MEMORY (-5)
 #define LINMIN_ERR_LIBRARY_NONFINITE (-6) /* A contains NaN or Inf */
+#define LINMIN_ERR_COVARIANCE (-7)        /* the noise covariance is not finite / not positive definite */
 #define LINMIN_WARN_RANK_DEFICIENT 1      /* R > L: minimiser may be non-unique (PAPER.md:92 asks R <= L) */
 
 #define LINMIN_MAX_R 256
 #define LINMIN_MAX_L 512
 
-/* constraint (sto / slo / pos options of IPLS) */
+/* constraint (sto / slo / pos options of IPLS).  A property of the library handle:
+ * linmin_library_create reads it from opts, linmin_unmix_lib requires the same value (or opts == NULL). */
 #define LINMIN_CONSTRAINT_SUM_TO_ONE 0        /* eq. 3 + eq. 4: the hot path */
-#define LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE 1 /* not implemented yet */
-#define LINMIN_CONSTRAINT_POSITIVITY_ONLY 2    /* not implemented yet */
+#define LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE 1 /* a >= 0, sum a <= 1: sum-to-one with a slack (all-zero) endmember,
+                                                  added BEFORE the centring; the slack is not returned */
+#define LINMIN_CONSTRAINT_POSITIVITY_ONLY 2    /* eq. 3 only (NNLS): no centring, no equality constraint */
 
-/* weighting (eq. 5-6) */
+/* weighting (sec. 2.3, eq. 5-6: the renormalised problem).  Also a property of the handle.
+ * With a covariance, eq. 2 is solved on the whitened data X' = X.L, S' = S.L (C^-1 = L.L^T); the `sigma`
+ * argument of the solve calls is then ignored: coeff_sigma is the projected inverse Hessian of the whitened
+ * problem (unit noise) and resid is the RMS of the WHITENED residual, sqrt(r'C^-1 r / L) (about 1 when the
+ * model fits to the noise; reading R17). */
 #define LINMIN_WEIGHTING_NONE 0               /* unweighted fit; sigma used for propagation only */
-#define LINMIN_WEIGHTING_SHARED_COVARIANCE 1  /* not implemented yet */
+#define LINMIN_WEIGHTING_SHARED_COVARIANCE 1  /* opts->cov = L x L covariance matrix (row-major, symmetric pos. def.) */
+#define LINMIN_WEIGHTING_SHARED_DIAGONAL 2    /* opts->cov = L per-channel noise standard deviations (C = diag(cov^2)) */
 
 /* per-pixel info word (opts->info_out): flags in bits 0-7, then three counters */
 #define LINMIN_INFO_CONVERGED 0x01      /* IPLS met its stopping rule */
@@ -109,6 +117,8 @@ typedef struct linmin_opts {
     int32_t *info_out;          /* optional int32[N] (device pointer; host pointer for linmin_unmix_host) */
     int32_t deterministic;      /* results never depend on tiling or scheduling; kept for ABI, always on */
     int32_t reserved;
+    const float *cov;           /* weighting != NONE: the shared noise covariance (device pointer; host pointer for
+                                   linmin_unmix_host); read by linmin_library_create / linmin_unmix only */
 } linmin_opts;
 
 typedef struct linmin_library linmin_library; /* opaque: precomputed per-library data on the device */
@@ -118,7 +128,8 @@ typedef struct linmin_library linmin_library; /* opaque: precomputed per-library
  * matrix) -- all computed by kernels on opts->stream.  A is a DEVICE pointer (copied; the caller may
  * free it afterwards).  Synchronises the stream ONCE, at the end, to read the device flag that says
  * whether A is finite.  Returns LINMIN_OK, LINMIN_WARN_RANK_DEFICIENT (handle valid) or an error
- * (*lib = NULL; LINMIN_ERR_LIBRARY_NONFINITE for NaN/Inf in A).  Only opts->stream is read. */
+ * (*lib = NULL; LINMIN_ERR_LIBRARY_NONFINITE for NaN/Inf in A, LINMIN_ERR_COVARIANCE for a covariance that is not
+ * positive definite).  opts->stream, constraint, weighting and cov are read. */
 int linmin_library_create(const float *A, int32_t L, int32_t R, const linmin_opts *opts,
                           linmin_library **lib);
 

@@ -27,6 +27,8 @@ struct LibView {
     const double *G64;  // R x R fp64, A'A + t 11' (uncentred, exact data; t: precompute.cuh; drives the finish)
     const float *scal;  // device scalars of the precompute: [0] gdmax = max_i Gc[i][i] (1 if that is 0), [1] sum of Giq
     const int *flags;   // device word: bit 0 = the library holds a non-finite value (every kernel then returns at once)
+    int cons;           // 1: the coefficients sum to one (sto, and slo through its slack endmember); 0: positivity only
+                        // (pos: no equality constraint, nu == 0, library not centred, G64 not shifted)
     const float *Gi;    // R x R fp32, (Gc + 1e-4 gdmax I)^-1 (start point of IPLS: regularised sum-constrained LS)
     const float *Giq;   // R, row sums of Gi
 };

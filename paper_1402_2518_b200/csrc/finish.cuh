@@ -38,7 +38,7 @@ __host__ __device__ inline size_t finish_warp_bytes(int L, int R, int KMAX) {
 // state[i]: 0 free, 1 in F, 2 blocked (rejected as rank-deficient or degenerate tie)
 __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams prm, int KMAX) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    if (lib.flags[0] & 1) return;
+    if (lib.flags[0]) return;
     const int L = lib.L, R = lib.R;
     const int warps = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned char *basep = smem_raw + (size_t)warp * ((finish_warp_bytes(L, R, KMAX) + 15) & ~(size_t)15);
@@ -53,6 +53,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
     const float *A = lib.A;      // by channel: the multiplier pass walks the endmembers across the lanes
     const float *At = lib.At;    // by endmember: every pass over the channels of one member reads consecutive addresses
     const int max_pivots = 4 * KMAX + 8;
+    const bool cons = lib.cons != 0;      // false: positivity only (no equality constraint; the empty support is feasible)
 
     for (int64_t p = (int64_t)blockIdx.x * warps + warp; p < prm.N; p += (int64_t)gridDim.x * warps) {
         float *cout = prm.coeffs + p * R;
@@ -91,7 +92,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
             if (in && pos < KMAX) { idx[pos] = i; aF[pos] = (double)ai; state[i] = 1; }
             k = min(KMAX, k + __popc(m));
         }
-        if (k == 0) {   // (can not happen for a point on the simplex; be safe) take the largest entry
+        if (k == 0 && cons) {   // (can not happen for a point on the simplex; be safe) take the largest entry
             float best = warp_max(amax);
             unsigned m = __ballot_sync(0xffffffffu, amax == best);
             int src = __ffs(m) - 1;
@@ -100,7 +101,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
             k = 1;
         }
         __syncwarp();
-        {   // normalise onto the simplex
+        if (cons) {   // normalise onto the simplex
             double s = 0.0;
             for (int j = lane; j < k; j += 32) s += aF[j];
             s = warp_sum(s);
@@ -146,8 +147,8 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
                 }
                 --k; last_added = -1;
                 __syncwarp();
-                if (k == 0) { fallback = true; break; }
-                if (arej != 0.0) {
+                if (k == 0 && cons) { fallback = true; break; }
+                if (arej != 0.0 && cons) {
                     double s = 0.0;
                     for (int j = lane; j < k; j += 32) s += aF[j];
                     s = warp_sum(s);
@@ -185,7 +186,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
             double sp = 0.0;
             for (int j = lane; j < k; j += 32) sp += atry[j];
             sp = warp_sum(sp);
-            double mu = (sp - (1.0 - suma)) / sq;
+            double mu = cons ? (sp - (1.0 - suma)) / sq : 0.0;
             double amin = INFINITY;
             for (int j = lane; j < k; j += 32) {
                 double an = aF[j] + atry[j] - mu * q[j];
@@ -222,12 +223,12 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
                             idx[nk] = idx[j]; aF[nk] = an; s += an; ++nk;
                         }
                     }
-                    for (int j = 0; j < nk; ++j) aF[j] /= s;
+                    if (cons) for (int j = 0; j < nk; ++j) aF[j] /= s;
                 }
                 k = __shfl_sync(0xffffffffu, nk, 0);
                 last_added = -1;
                 __syncwarp();
-                if (k == 0 || ++pivots > max_pivots) { fallback = true; break; }
+                if ((k == 0 && cons) || ++pivots > max_pivots) { fallback = true; break; }
                 continue;
             }
             // ---- accept; residual and gradient at the new point
@@ -247,6 +248,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
                 s = warp_sum(s);
                 nu += s * aF[j];
             }
+            if (!cons) nu = 0.0;
             // multipliers lambda_i = nu - A_i'r off the support (fp32 dot products of the fp64 residual)
             float lmin = INFINITY; int jmin = -1; float gmax = 0.0f;
             for (int i = lane; i < R; i += 32) {
@@ -313,7 +315,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
                 const float qnan = __int_as_float(0x7fc00000);
                 for (int i = lane; i < R; i += 32) sout[i] = qnan;
                 info |= LINMIN_INFO_BAD_SIGMA;
-            } else if (k > 1 && !fallback) {
+            } else if (k > (cons ? 1 : 0) && !fallback) {
                 // Lf, dinv, q hold the factor of the FINAL support (last loop pass ended in `break`
                 // right after an accepted solve).  W = L^-1 in place (column by column from the end).
                 double sq = 0.0;
@@ -339,7 +341,7 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
                             double wmj = (m == j) ? dinv[j] : Lf[cm(k, m, j)];
                             s += wmi * wmj;
                         }
-                        Hs[cm(k, i, j)] = (float)(s - q[i] * q[j] / sq);
+                        Hs[cm(k, i, j)] = (float)(cons ? s - q[i] * q[j] / sq : s);     // pos: H = K, no projection
                     }
                 __syncwarp();
                 const float *sg = prm.has_sigma ? prm.sigma + p * prm.sigma_stride : nullptr;

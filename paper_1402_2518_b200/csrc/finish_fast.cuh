@@ -70,7 +70,7 @@ __global__ void __launch_bounds__(512, 1)
 finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter,
                    const unsigned int *__restrict__ list /* NULL: all pixels; else [0] = count, [1 + i] = pixel */) {
     using namespace ff;
-    if ((list && list[0] == 0u) || (lib.flags[0] & 1)) return;
+    if ((list && list[0] == 0u) || lib.flags[0]) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int L = lib.L, R = lib.R;
     const int AST = ast(LV);

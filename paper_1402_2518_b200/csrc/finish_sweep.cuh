@@ -95,7 +95,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
     constexpr int RS = 32 * LQ;         // library row stride (elements)
     constexpr int IT = (LQ <= 4) ? 4 : 2;   // J rows per tile
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    if (lib.flags[0] & 1) return;
+    if (lib.flags[0]) return;
     const int L = lib.L, R = lib.R;
     double *G64s = (double *)smem_raw;                                    // [RP][GS]
     float *At32 = (float *)(smem_raw + (size_t)RP * GS * 8);              // [RP][32 LQ]: library rows, fp32 (widened on the fly:

@@ -278,7 +278,7 @@ template <int TEAM>
 __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolveParams prm) {
     using Ops = TeamOps<TEAM>;
     extern __shared__ __align__(16) float smem[];
-    if (lib.flags[0] & 1) return;      // non-finite library: the caller is told (status or poisoned outputs)
+    if (lib.flags[0]) return;      // non-finite library: the caller is told (status or poisoned outputs)
     const float gdmax = lib.scal[0];
     const int L = lib.L, R = lib.R;
     const int teams_per_cta = blockDim.x / TEAM;
@@ -290,6 +290,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
           *Mp = (TEAM == 32) ? base + ipls_generic_vec_floats(L, R) : red + 64;
     const float fR = (float)R;
     const float tau = 0.995f;
+    const bool cons = lib.cons != 0;      // false: positivity only -- no nu, no primal equality residual
 
     for (int64_t p = (int64_t)blockIdx.x * teams_per_cta + team; p < prm.N;
          p += (int64_t)gridDim.x * teams_per_cta) {
@@ -331,7 +332,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
                 u[i] = s; sx += s; sq += lib.Giq[i];
             }
             sx = Ops::sum(sx, red); sq = Ops::sum(sq, red);
-            const float mu0 = (sx - 1.0f) / sq;
+            const float mu0 = cons ? (sx - 1.0f) / sq : 0.0f;
             for (int i = t; i < R; i += TEAM) u[i] = fmaf(-mu0, lib.Giq[i], u[i]);       // x
             Ops::sync();
             float gx = 0.0f, mnx = INFINITY, mng = INFINITY;
@@ -345,7 +346,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
                 gx = fmaf(gi, u[i], gx); mnx = fminf(mnx, u[i]); mng = fminf(mng, gi);
             }
             gx = Ops::sum(gx, red); mnx = Ops::min(mnx, red); mng = Ops::min(mng, red);
-            nu = -gx;
+            nu = cons ? -gx : 0.0f;
             const float dp = fmaxf(-mnx, 0.0f), dd = fmaxf(-(mng + nu), 0.0f);
             float xl = 0.0f, sl = 0.0f, sxx = 0.0f;
             for (int i = t; i < R; i += TEAM) {
@@ -362,7 +363,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
                 sa += ai; lm = fmaxf(lm, li);
             }
             sa = Ops::sum(sa, red); lam0 = Ops::max(lm, red);
-            const float rsa = 1.0f / sa;
+            const float rsa = cons ? 1.0f / sa : 1.0f;      // pos: the point is not normalised
             const bool ok = (lam0 > 0.0f) && isfinite(lam0) && isfinite(sa) && isfinite(rsa);
             if (!ok) { lam0 = fmaxf(bmax, 1e-3f * gdmax); nu = 0.0f; }
             for (int i = t; i < R; i += TEAM) {
@@ -390,7 +391,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
             rdmax = Ops::max(rdmax, red);
             suma = Ops::sum(suma, red);
             gap = Ops::sum(gap, red);
-            const float rp = suma - 1.0f;
+            const float rp = cons ? suma - 1.0f : 0.0f;
             if (gap <= prm.gap_tol * sc && rdmax <= prm.feas_tol * sc && fabsf(rp) <= prm.feas_tol) {
                 flags |= LINMIN_INFO_CONVERGED;
                 break;
@@ -429,7 +430,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
             for (int i = t; i < R; i += TEAM) { su += u[i]; sv += v[i]; }
             su = Ops::sum(su, red);
             sv = Ops::sum(sv, red);
-            float dnu = (su + rp) / sv;
+            float dnu = cons ? (su + rp) / sv : 0.0f;
             float ap = INFINITY, ad = INFINITY;
             for (int i = t; i < R; i += TEAM) {
                 float dai = u[i] - v[i] * dnu;
@@ -457,7 +458,7 @@ __global__ void __launch_bounds__(256) ipls_generic_kernel(LibView lib, SolvePar
             su = 0.0f;
             for (int i = t; i < R; i += TEAM) su += u[i];
             su = Ops::sum(su, red);
-            dnu = (su + rp) / sv;
+            dnu = cons ? (su + rp) / sv : 0.0f;
             ap = INFINITY; ad = INFINITY;
             for (int i = t; i < R; i += TEAM) {
                 float dai = u[i] - v[i] * dnu;

@@ -87,7 +87,7 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
                 unsigned int *__restrict__ counter) {
     using namespace q32;
     extern __shared__ __align__(16) float smem[];
-    if (lib.flags[0] & 1) return;      // non-finite library: the caller is told (status or poisoned outputs)
+    if (lib.flags[0]) return;      // non-finite library: the caller is told (status or poisoned outputs)
     float *Gp = smem;                                             // [32][GST]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     float *wbase = Gp + R * GST + (size_t)warp * (8 * PIXF + QD * REC + QD);

@@ -18,6 +18,7 @@
 #include "ipls_generic.cuh"
 #include "ipls_q32.cuh"
 #include "precompute.cuh"
+#include "whiten.cuh"
 
 using namespace linmin;
 
@@ -30,7 +31,11 @@ inline bool finish_sweep_supported(int L, int R) { return R <= 32 && L <= 256; }
 }  // namespace linmin
 
 struct linmin_library {
-    int L = 0, R = 0;
+    int L = 0, R = 0;                // the caller's sizes
+    int Ri = 0;                      // endmembers the kernels see: R, or R + 1 with the slack endmember of slo
+    int constraint = LINMIN_CONSTRAINT_SUM_TO_ONE, weighting = LINMIN_WEIGHTING_NONE;
+    float *W = nullptr;              // weighting: L x L whitening matrix (fp32, lower triangular), Y' = Y W'
+    double *Wd = nullptr, *Cd = nullptr;
     int device = 0;
     int sm_count = 0;
     cudaStream_t stream = nullptr;   // stream the handle was created on (frees are ordered on it)
@@ -106,6 +111,8 @@ int cuda_status(cudaError_t e) {
 
 struct Resolved {
     cudaStream_t stream;
+    int constraint, weighting;
+    const float *cov;
     int64_t ldY, sstride;
     int max_iter;
     float gap_tol, feas_tol;
@@ -115,17 +122,14 @@ struct Resolved {
 int resolve_opts(const linmin_opts *o, int L, Resolved *r) {
     r->stream = nullptr; r->ldY = L; r->sstride = 0; r->max_iter = 50;
     r->gap_tol = 1e-7f; r->feas_tol = 3e-5f; r->info = nullptr;   // measured optimum of IPLS + finish time
+    r->constraint = LINMIN_CONSTRAINT_SUM_TO_ONE; r->weighting = LINMIN_WEIGHTING_NONE; r->cov = nullptr;
     if (!o) return LINMIN_OK;
     if (o->struct_size != sizeof(linmin_opts)) return LINMIN_ERR_INVALID_ARGUMENT;
-    if (o->constraint != LINMIN_CONSTRAINT_SUM_TO_ONE) {
-        if (o->constraint == LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE || o->constraint == LINMIN_CONSTRAINT_POSITIVITY_ONLY)
-            return LINMIN_ERR_NOT_IMPLEMENTED;
+    if (o->constraint < LINMIN_CONSTRAINT_SUM_TO_ONE || o->constraint > LINMIN_CONSTRAINT_POSITIVITY_ONLY)
         return LINMIN_ERR_INVALID_ARGUMENT;
-    }
-    if (o->weighting != LINMIN_WEIGHTING_NONE) {
-        if (o->weighting == LINMIN_WEIGHTING_SHARED_COVARIANCE) return LINMIN_ERR_NOT_IMPLEMENTED;
+    if (o->weighting < LINMIN_WEIGHTING_NONE || o->weighting > LINMIN_WEIGHTING_SHARED_DIAGONAL)
         return LINMIN_ERR_INVALID_ARGUMENT;
-    }
+    r->constraint = o->constraint; r->weighting = o->weighting; r->cov = o->cov;
     r->stream = (cudaStream_t)o->stream;
     if (o->ldY != 0) { if (o->ldY < L) return LINMIN_ERR_INVALID_ARGUMENT; r->ldY = o->ldY; }
     if (o->sigma_pixel_stride != 0) {
@@ -151,7 +155,8 @@ int check_sizes(int64_t N, int L, int R) {
 
 LibView view_of(const linmin_library *lib) {
     LibView v;
-    v.L = lib->L; v.R = lib->R; v.A = lib->A; v.At = lib->At; v.Ac = lib->Ac; v.c = lib->c; v.Gc = lib->Gc;
+    v.cons = lib->constraint != LINMIN_CONSTRAINT_POSITIVITY_ONLY;
+    v.L = lib->L; v.R = lib->Ri; v.A = lib->A; v.At = lib->At; v.Ac = lib->Ac; v.c = lib->c; v.Gc = lib->Gc;
     v.G64 = lib->G64; v.scal = lib->scal; v.flags = lib->flags; v.Gi = lib->Gi; v.Giq = lib->Giq;
     return v;
 }
@@ -191,21 +196,44 @@ void note_use(const linmin_library *lib, cudaStream_t stream) {
 
 int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
                  const Resolved &o, float *coeffs, float *csig, float *resid) {
-    const int L = lib->L, R = lib->R;
+    const int L = lib->L, R = lib->Ri;      // R: the endmembers the kernels see (slack included)
+    const bool cons = lib->constraint != LINMIN_CONSTRAINT_POSITIVITY_ONLY;
     LibView lv = view_of(lib);
+    struct FreeV { void *p; cudaStream_t s; ~FreeV() { if (p) cudaFreeAsync(p, s); } };
+    int launches = 0;
+    if (lib->timing) CK(cudaEventRecord(lib->ev[0], o.stream));
+    int64_t ldY = o.ldY, sstride = o.sstride;
+    // ---- renormalised problem (eq. 6): Y' = Y W' into a workspace, then the unweighted path on
+    //      (A', Y') with unit noise
+    float *Yw = nullptr;
+    if (lib->weighting != LINMIN_WEIGHTING_NONE) {
+        CK(staging_alloc((void **)&Yw, (size_t)N * L * sizeof(float), o.stream));
+        CK(launch_whiten_spectra(Y, o.ldY, N, L, lib->W, lib->weighting == LINMIN_WEIGHTING_SHARED_DIAGONAL, Yw,
+                                 lib->sm_count, o.stream));
+        ++launches;
+        Y = Yw; ldY = L; sigma = nullptr; sstride = 0;
+    }
+    FreeV free_yw{Yw, o.stream};
+    // ---- slo: the kernels work on R + 1 endmembers; their outputs go to internal arrays, the slack is stripped
+    float *ci = nullptr, *si = nullptr;
+    float *coeffs_user = coeffs, *csig_user = csig;
+    if (R != lib->R) {
+        CK(staging_alloc((void **)&ci, (size_t)N * R * sizeof(float), o.stream));
+        if (csig) CK(staging_alloc((void **)&si, (size_t)N * R * sizeof(float), o.stream));
+        coeffs = ci; csig = csig ? si : nullptr;
+    }
+    FreeV free_ci{ci, o.stream}, free_si{si, o.stream};
     SolveParams prm;
-    prm.Y = Y; prm.sigma = sigma; prm.N = N; prm.ldY = o.ldY; prm.sigma_stride = o.sstride;
+    prm.Y = Y; prm.sigma = sigma; prm.N = N; prm.ldY = ldY; prm.sigma_stride = sstride;
     prm.has_sigma = sigma != nullptr;
     prm.max_iter = o.max_iter; prm.gap_tol = o.gap_tol; prm.feas_tol = o.feas_tol;
     prm.coeffs = coeffs; prm.coeff_sigma = csig; prm.resid = resid; prm.info = o.info;
-    int launches = 0;
-    if (lib->timing) CK(cudaEventRecord(lib->ev[0], o.stream));
 
     // ---- K1: projection + IPLS
     // per-call workspace, because one handle may serve several streams: the work counters of the persistent
     // kernels (8 words), then two pixel lists of finish_sweep (count + one entry per pixel each): the overflow
     // list (supports above 16) and the repair list (pixels whose support changes after the first round)
-    const bool use_f8 = finish_sweep_supported(L, R);
+    const bool use_f8 = cons && finish_sweep_supported(L, R);
     unsigned int *ws = nullptr;
     const size_t ws_words = 8 + (use_f8 ? 2 * ((size_t)N + 1) : 0);
     CK(staging_alloc((void **)&ws, ws_words * sizeof(unsigned int), o.stream));
@@ -213,7 +241,7 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     CK(cudaMemsetAsync(ws, 0, std::min<size_t>(9, ws_words) * sizeof(unsigned int), o.stream));
     unsigned int *counters = ws, *overflow = ws + 8, *repair = ws + 8 + ((size_t)N + 1);
     if (use_f8) CK(cudaMemsetAsync(repair, 0, sizeof(unsigned int), o.stream));
-    if (R == 32 && start_r32_warps(L) > 0) {
+    if (cons && R == 32 && start_r32_warps(L) > 0) {
         // K0 (projection + start point, one record per pixel) and K1 (the iteration), in chunks of 2^21 pixels
         // so that the record workspace stays at 0.8 GB whatever N is
         const int64_t chunk = (int64_t)1 << 21;
@@ -260,7 +288,7 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
         // pixels whose support outgrew finish_sweep (none on the synthetic cubes): one-warp-per-pixel kernel
         CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, o.stream));
         ++launches;
-    } else if (finish_fast_supported(L, R)) {
+    } else if (cons && finish_fast_supported(L, R)) {
         CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, nullptr, o.stream));
         ++launches;
     } else {
@@ -275,6 +303,12 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
         CK(cudaGetLastError());
         ++launches;
     }
+    if (R != lib->R) {
+        const int grid = (int)std::min<int64_t>((N * lib->R + 255) / 256, (int64_t)lib->sm_count * 16);
+        strip_slack_kernel<<<grid, 256, 0, o.stream>>>(ci, si, N, lib->R, R, coeffs_user, csig_user, o.info);
+        CK(cudaGetLastError());
+        ++launches;
+    }
     if (lib->timing) { CK(cudaEventRecord(lib->ev[2], o.stream)); lib->timed.store(true); }
     lib->last_launches.store(launches);
     note_use(lib, o.stream);
@@ -284,15 +318,23 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
 // Once-per-library precompute, all of it on the device and enqueued on `stream`: copy of A,
 // centred library, transposed copy, Gram matrices, start-point data.  No host round trip; `wait_check` adds the
 // ONE synchronisation linmin_library_create documents (to return LINMIN_ERR_LIBRARY_NONFINITE).
-int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool A_on_host, bool wait_check,
-                        linmin_library **out) {
+int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool on_host, bool wait_check,
+                        int constraint, int weighting, const float *cov, linmin_library **out) {
     *out = nullptr;
+    if (weighting != LINMIN_WEIGHTING_NONE && !cov) return LINMIN_ERR_INVALID_ARGUMENT;
+    const int Ri = (constraint == LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE) ? R + 1 : R;
+    if (Ri > LINMIN_MAX_R) return LINMIN_ERR_UNSUPPORTED_SIZE;
+    const bool cons = constraint != LINMIN_CONSTRAINT_POSITIVITY_ONLY;
     int dev = 0;
     CK(cudaGetDevice(&dev));
     linmin_library *lib = new (std::nothrow) linmin_library();
     if (!lib) return LINMIN_ERR_OUT_OF_MEMORY;
-    lib->L = L; lib->R = R; lib->device = dev; lib->stream = stream;
+    lib->L = L; lib->R = R; lib->Ri = Ri; lib->constraint = constraint; lib->weighting = weighting;
+    lib->device = dev; lib->stream = stream;
+    float *Araw = nullptr, *covd = nullptr;       // device copies of the caller's arrays (released below)
     auto fail = [&](int code) {
+        if (Araw) cudaFreeAsync(Araw, stream);
+        if (covd) cudaFreeAsync(covd, stream);
         linmin_library_destroy(lib);
         return code;
     };
@@ -302,41 +344,62 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
         if (e__ != cudaSuccess) { (void)cudaGetLastError(); return fail(cuda_status(e__)); } \
     } while (0)
     CKF(cudaDeviceGetAttribute(&lib->sm_count, cudaDevAttrMultiProcessorCount, dev));
-    const size_t LR = (size_t)L * R, RR = (size_t)R * R;
+    const size_t LR = (size_t)L * Ri, RR = (size_t)Ri * Ri, LL = (size_t)L * L;
     CKF(cudaMallocAsync((void **)&lib->A, LR * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->At, LR * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->Ac, LR * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->c, (size_t)L * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->Gc, RR * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->Gi, RR * sizeof(float), stream));
-    CKF(cudaMallocAsync((void **)&lib->Giq, (size_t)R * sizeof(float), stream));
+    CKF(cudaMallocAsync((void **)&lib->Giq, (size_t)Ri * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->scal, 4 * sizeof(float), stream));
     CKF(cudaMallocAsync((void **)&lib->G64, RR * sizeof(double), stream));
     CKF(cudaMallocAsync((void **)&lib->W64, RR * sizeof(double), stream));
     CKF(cudaMallocAsync((void **)&lib->flags, sizeof(int), stream));
     CKF(cudaMemsetAsync(lib->flags, 0, sizeof(int), stream));
-    CKF(cudaMemcpyAsync(lib->A, A, LR * sizeof(float), A_on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, stream));
-    {
-        int block = 256, grid = (L * 32 + block - 1) / block;
-        center_library_kernel<<<grid, block, 0, stream>>>(lib->A, L, R, lib->Ac, lib->c, lib->flags);
-        CKF(cudaGetLastError());
-        transpose_library_kernel<<<(int)((LR + block - 1) / block), block, 0, stream>>>(lib->A, L, R, lib->At);
-        CKF(cudaGetLastError());
-        grid = (int)((RR + block - 1) / block);
-        gram_kernel<<<grid, block, 0, stream>>>(lib->A, lib->Ac, L, R, lib->G64, lib->Gc);
-        CKF(cudaGetLastError());
-        // start point data of IPLS: inverse of the regularised centred Gram matrix, its row sums, gdmax
-        start_data_kernel<<<1, 1024, 0, stream>>>(lib->Gc, R, lib->W64, lib->Gi, lib->Giq, lib->scal, lib->G64, 1);
+    CKF(cudaMallocAsync((void **)&Araw, (size_t)L * R * sizeof(float), stream));
+    CKF(cudaMemcpyAsync(Araw, A, (size_t)L * R * sizeof(float), on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, stream));
+    if (weighting != LINMIN_WEIGHTING_NONE) {
+        // renormalised problem: C = Rc Rc', W = Rc^-1, A' = W A
+        const size_t ncov = (weighting == LINMIN_WEIGHTING_SHARED_DIAGONAL) ? (size_t)L : LL;
+        CKF(cudaMallocAsync((void **)&covd, ncov * sizeof(float), stream));
+        CKF(cudaMemcpyAsync(covd, cov, ncov * sizeof(float), on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, stream));
+        CKF(cudaMallocAsync((void **)&lib->W, LL * sizeof(float), stream));
+        CKF(cudaMallocAsync((void **)&lib->Wd, LL * sizeof(double), stream));
+        CKF(cudaMallocAsync((void **)&lib->Cd, LL * sizeof(double), stream));
+        whitening_matrix_kernel<<<1, 1024, 0, stream>>>(covd, weighting == LINMIN_WEIGHTING_SHARED_DIAGONAL ? 1 : 2, L,
+                                                        lib->Cd, lib->Wd, lib->W, lib->flags);
         CKF(cudaGetLastError());
     }
+    {
+        int block = 256;
+        // the library the kernels see: whitened, with the slack endmember of slo as a last, all-zero column
+        whiten_library_kernel<<<(int)((LR + block - 1) / block), block, 0, stream>>>(Araw, L, R, Ri, lib->Wd, lib->A);
+        CKF(cudaGetLastError());
+        int grid = (L * 32 + block - 1) / block;
+        // pos: no centring (it is only valid under sum a = 1) and no shift of the fp64 Gram matrix
+        center_library_kernel<<<grid, block, 0, stream>>>(lib->A, Araw, L, Ri, R, cons ? 1 : 0, lib->Ac, lib->c, lib->flags);
+        CKF(cudaGetLastError());
+        transpose_library_kernel<<<(int)((LR + block - 1) / block), block, 0, stream>>>(lib->A, L, Ri, lib->At);
+        CKF(cudaGetLastError());
+        grid = (int)((RR + block - 1) / block);
+        gram_kernel<<<grid, block, 0, stream>>>(lib->A, lib->Ac, L, Ri, lib->G64, lib->Gc);
+        CKF(cudaGetLastError());
+        // start point data of IPLS: inverse of the regularised centred Gram matrix, its row sums, gdmax
+        start_data_kernel<<<1, 1024, 0, stream>>>(lib->Gc, Ri, lib->W64, lib->Gi, lib->Giq, lib->scal, lib->G64, cons ? 1 : 0);
+        CKF(cudaGetLastError());
+    }
+    cudaFreeAsync(Araw, stream); Araw = nullptr;
+    if (covd) { cudaFreeAsync(covd, stream); covd = nullptr; }
     if (wait_check) {
         int hflags = 0;
         CKF(cudaMemcpyAsync(&hflags, lib->flags, sizeof(int), cudaMemcpyDeviceToHost, stream));
         CKF(cudaStreamSynchronize(stream));
         if (hflags & 1) return fail(LINMIN_ERR_LIBRARY_NONFINITE);
+        if (hflags & 2) return fail(LINMIN_ERR_COVARIANCE);
     }
     *out = lib;
-    return (R > L) ? LINMIN_WARN_RANK_DEFICIENT : LINMIN_OK;
+    return (Ri > L) ? LINMIN_WARN_RANK_DEFICIENT : LINMIN_OK;
 #undef CKF
 }
 
@@ -358,10 +421,11 @@ const char *linmin_strerror(int code) {
         case LINMIN_OK: return "ok";
         case LINMIN_ERR_INVALID_ARGUMENT: return "invalid argument";
         case LINMIN_ERR_UNSUPPORTED_SIZE: return "unsupported size (R > 256 or L > 512)";
-        case LINMIN_ERR_NOT_IMPLEMENTED: return "option not implemented";
+        case LINMIN_ERR_NOT_IMPLEMENTED: return "option not implemented (unused: every option of linmin.h is built)";
         case LINMIN_ERR_CUDA: return "CUDA runtime error (no device, or a failed call)";
         case LINMIN_ERR_OUT_OF_MEMORY: return "out of device memory";
         case LINMIN_ERR_LIBRARY_NONFINITE: return "library A contains a non-finite value";
+        case LINMIN_ERR_COVARIANCE: return "noise covariance is not finite or not positive definite";
         case LINMIN_WARN_RANK_DEFICIENT: return "warning: R > L, the minimiser may be non-unique";
         default: return "unknown status code";
     }
@@ -373,12 +437,10 @@ int linmin_library_create(const float *A, int32_t L, int32_t R, const linmin_opt
     if (!A) return LINMIN_ERR_INVALID_ARGUMENT;
     int rc = check_sizes(0, L, R);
     if (rc != LINMIN_OK) return rc;
-    cudaStream_t stream = nullptr;
-    if (opts) {
-        if (opts->struct_size != sizeof(linmin_opts)) return LINMIN_ERR_INVALID_ARGUMENT;
-        stream = (cudaStream_t)opts->stream;
-    }
-    return library_create_impl(A, L, R, stream, false, true, lib);
+    Resolved o;
+    rc = resolve_opts(opts, L, &o);
+    if (rc != LINMIN_OK) return rc;
+    return library_create_impl(A, L, R, o.stream, false, true, o.constraint, o.weighting, o.cov, lib);
 }
 
 void linmin_library_destroy(linmin_library *lib) {
@@ -393,7 +455,8 @@ void linmin_library_destroy(linmin_library *lib) {
         }
         lib->n_use = 0;
     }
-    void *bufs[] = {lib->A, lib->At, lib->Ac, lib->c, lib->Gc, lib->Gi, lib->Giq, lib->scal, lib->G64, lib->W64, lib->flags};
+    void *bufs[] = {lib->A, lib->At, lib->Ac, lib->c, lib->Gc, lib->Gi, lib->Giq, lib->scal, lib->G64, lib->W64, lib->flags,
+                    lib->W, lib->Wd, lib->Cd};
     for (void *q : bufs) if (q) cudaFreeAsync(q, s);
     for (int i = 0; i < 3; ++i) if (lib->ev[i]) cudaEventDestroy(lib->ev[i]);
     (void)cudaGetLastError();
@@ -429,6 +492,8 @@ int linmin_unmix_lib(const linmin_library *lib, const float *Y, const float *sig
     Resolved o;
     int rc = resolve_opts(opts, lib->L, &o);
     if (rc != LINMIN_OK) return rc;
+    // constraint and weighting are properties of the handle: opts must agree with it (or be NULL)
+    if (opts && (o.constraint != lib->constraint || o.weighting != lib->weighting)) return LINMIN_ERR_INVALID_ARGUMENT;
     if (N >= ((int64_t)1 << 32)) return LINMIN_ERR_UNSUPPORTED_SIZE;
     if (N == 0) { lib->last_launches.store(0); return LINMIN_OK; }
     if (!Y || !coeffs_out) return LINMIN_ERR_INVALID_ARGUMENT;
@@ -451,7 +516,7 @@ int linmin_unmix(const float *A, const float *Y, const float *sigma, int64_t N, 
     // everything is enqueued on the caller's stream and the call returns: no synchronisation, no host arithmetic.
     // A non-finite library can therefore not be reported through the status: the solve kernels return at once on
     // the device flag and the outputs are poisoned instead (NaN, LINMIN_INFO_LIBRARY_NONFINITE).
-    int wrc = library_create_impl(A, L, R, o.stream, false, false, &lib);
+    int wrc = library_create_impl(A, L, R, o.stream, false, false, o.constraint, o.weighting, o.cov, &lib);
     if (wrc < 0) return wrc;
     rc = LINMIN_OK;
     if (N > 0) {
@@ -503,7 +568,7 @@ int linmin_unmix_host(const float *A, const float *Y, const float *sigma, int64_
         cudaError_t e__ = (call);                                                   \
         if (e__ != cudaSuccess) { (void)cudaGetLastError(); cleanup(); return cuda_status(e__); } \
     } while (0)
-    wrc = library_create_impl(A, L, R, nullptr, true, true, &lib);
+    wrc = library_create_impl(A, L, R, nullptr, true, true, o.constraint, o.weighting, o.cov, &lib);
     if (wrc < 0) { lib = nullptr; return wrc; }
     if (N == 0) { cleanup(); return wrc; }
     const bool per_pixel_sigma = sigma && o.sstride != 0;

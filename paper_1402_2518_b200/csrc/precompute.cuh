@@ -19,24 +19,21 @@ __global__ void transpose_library_kernel(const float *__restrict__ A, int L, int
     At[(size_t)r * L + l] = A[e];
 }
 
-// one warp per channel l: c[l] = mean_r A[l][r] (fp64), Ac[l][r] = fl32(A[l][r] - c[l]).
-// flags[0] |= 1 when A holds a non-finite value.
-__global__ void center_library_kernel(const float *__restrict__ A, int L, int R, float *__restrict__ Ac,
-                                      float *__restrict__ c, int *__restrict__ flags) {
+// one warp per channel l: c[l] = mean_r A[l][r] (fp64), Ac[l][r] = fl32(A[l][r] - c[l]); center == 0 (pos option):
+// c = 0, Ac = A.  flags[0] |= 1 when the caller's library Araw (L x Rraw) holds a non-finite value.
+__global__ void center_library_kernel(const float *__restrict__ A, const float *__restrict__ Araw, int L, int R, int Rraw,
+                                      int center, float *__restrict__ Ac, float *__restrict__ c, int *__restrict__ flags) {
     int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     int lane = threadIdx.x & 31;
     if (warp >= L) return;
     const float *row = A + (size_t)warp * R;
     double s = 0.0;
     bool bad = false;
-    for (int r = lane; r < R; r += 32) {
-        float v = row[r];
-        bad |= !isfinite(v);
-        s += (double)v;
-    }
+    for (int r = lane; r < R; r += 32) s += (double)row[r];
+    for (int r = lane; r < Rraw; r += 32) bad |= !isfinite(Araw[(size_t)warp * Rraw + r]);
     s = warp_sum(s);
     if (__any_sync(0xffffffffu, bad) && lane == 0) atomicOr(flags, 1);
-    double mean = s / (double)R;
+    double mean = center ? s / (double)R : 0.0;
     for (int r = lane; r < R; r += 32) Ac[(size_t)warp * R + r] = (float)((double)row[r] - mean);
     if (lane == 0) c[warp] = (float)mean;
 }
@@ -141,7 +138,7 @@ start_data_kernel(const float *__restrict__ Gc, int R, double *__restrict__ W, f
 // call is overwritten with NaN and every info word with LINMIN_INFO_LIBRARY_NONFINITE (include/linmin.h).
 __global__ void poison_outputs_kernel(const int *__restrict__ flags, int64_t N, int R, float *__restrict__ coeffs,
                                       float *__restrict__ csig, float *__restrict__ resid, int32_t *__restrict__ info) {
-    if (!(flags[0] & 1)) return;
+    if (!flags[0]) return;
     const float qnan = __int_as_float(0x7fc00000);
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < N * R; e += stride) {

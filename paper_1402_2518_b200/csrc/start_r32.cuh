@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(s32::WARPS * 32, 1)
 start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, float *__restrict__ rec, int warps) {
     using namespace s32;
     extern __shared__ __align__(16) float smem[];
-    if (lib.flags[0] & 1) return;
+    if (lib.flags[0]) return;
     const int L = lib.L, Lp = lpad(L);
     float *Acp = smem;                          // [Lp][32] centred library, zero rows beyond L
     float *cv = Acp + (size_t)Lp * R;           // [Lp]

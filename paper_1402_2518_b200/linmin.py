@@ -21,6 +21,9 @@ ERR_NOT_IMPLEMENTED = -3
 ERR_CUDA = -4
 ERR_OUT_OF_MEMORY = -5
 ERR_LIBRARY_NONFINITE = -6
+ERR_COVARIANCE = -7
+CONSTRAINT_SUM_TO_ONE, CONSTRAINT_SUM_LOWER_THAN_ONE, CONSTRAINT_POSITIVITY_ONLY = 0, 1, 2
+WEIGHTING_NONE, WEIGHTING_SHARED_COVARIANCE, WEIGHTING_SHARED_DIAGONAL = 0, 1, 2
 WARN_RANK_DEFICIENT = 1
 
 INFO_CONVERGED = 0x01
@@ -43,7 +46,7 @@ class LinminOpts(ctypes.Structure):
                 ("constraint", ctypes.c_int32), ("weighting", ctypes.c_int32),
                 ("max_iter", ctypes.c_int32), ("gap_tol", ctypes.c_float),
                 ("feas_tol", ctypes.c_float), ("info_out", ctypes.c_void_p),
-                ("deterministic", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("deterministic", ctypes.c_int32), ("reserved", ctypes.c_int32), ("cov", ctypes.c_void_p)]
 
 
 class LinminError(RuntimeError):
@@ -113,7 +116,7 @@ def _dev_ptr(t, name, dtype=None):
 
 
 def _make_opts(stream=None, ldY=0, sigma_pixel_stride=0, constraint=0, weighting=0, max_iter=0,
-               gap_tol=0.0, feas_tol=0.0, info_ptr=None) -> LinminOpts:
+               gap_tol=0.0, feas_tol=0.0, info_ptr=None, cov_ptr=None) -> LinminOpts:
     o = LinminOpts()
     o.struct_size = ctypes.sizeof(LinminOpts)
     o.stream = stream
@@ -126,7 +129,20 @@ def _make_opts(stream=None, ldY=0, sigma_pixel_stride=0, constraint=0, weighting
     o.feas_tol = feas_tol
     o.info_out = info_ptr
     o.deterministic = 1
+    o.cov = cov_ptr
     return o
+
+
+def _weighting_of(cov, L, cuda, device=None):
+    """(weighting code, pointer) of a covariance argument: None, (L,) noise std, or (L, L) covariance matrix."""
+    torch = _torch()
+    if cov is None:
+        return WEIGHTING_NONE, None
+    if cov.dim() == 1:
+        _check_tensor(cov, "cov", (L,), torch.float32, cuda, device)
+        return WEIGHTING_SHARED_DIAGONAL, cov.data_ptr()
+    _check_tensor(cov, "cov", (L, L), torch.float32, cuda, device)
+    return WEIGHTING_SHARED_COVARIANCE, cov.data_ptr()
 
 
 def _sigma_stride(sigma, N, L):
@@ -144,15 +160,19 @@ def _sigma_stride(sigma, N, L):
 class Library:
     """linmin_library handle: once-per-library precompute kept on the device."""
 
-    def __init__(self, A):
+    def __init__(self, A, constraint=0, cov=None):
         torch = _torch()
         if A.dim() != 2:
             raise ValueError("A must be (L, R)")
         self.L, self.R = int(A.shape[0]), int(A.shape[1])
+        _check_tensor(A, "A", (self.L, self.R), torch.float32, True)
         self._h = ctypes.c_void_p()
         self.device = A.device
+        self.constraint = int(constraint)
+        self.weighting, cov_ptr = _weighting_of(cov, self.L, True, A.device)
         with torch.cuda.device(A.device):
-            o = _make_opts(stream=torch.cuda.current_stream().cuda_stream)
+            o = _make_opts(stream=torch.cuda.current_stream().cuda_stream, constraint=self.constraint,
+                           weighting=self.weighting, cov_ptr=cov_ptr)
             self.status = _check(load().linmin_library_create(_dev_ptr(A, "A"), self.L, self.R,
                                                               ctypes.byref(o), ctypes.byref(self._h)))
 
@@ -185,8 +205,9 @@ def trim_memory() -> None:
     _check(load().linmin_trim_memory())
 
 
-def library_create(A) -> Library:
-    return Library(A)
+def library_create(A, constraint=0, cov=None) -> Library:
+    """constraint: CONSTRAINT_*; cov: None | (L,) per-channel noise std | (L, L) covariance (the renormalised problem)."""
+    return Library(A, constraint, cov)
 
 
 def library_destroy(lib: Library) -> None:
@@ -247,8 +268,7 @@ def _alloc_outputs(N, R, device, want_sigma, want_resid, want_info, out):
 
 
 def unmix_lib(lib: Library, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=True,
-              out: Optional[dict] = None, max_iter=0, gap_tol=0.0, feas_tol=0.0, constraint=0,
-              weighting=0):
+              out: Optional[dict] = None, max_iter=0, gap_tol=0.0, feas_tol=0.0):
     """linmin_unmix_lib.  Y (N, L) CUDA float32 (rows may be strided); returns
     (coeffs, coeff_sigma, resid, info, status); enqueued on the current stream, not synchronised."""
     torch = _torch()
@@ -266,8 +286,8 @@ def unmix_lib(lib: Library, Y, sigma=None, *, want_sigma=True, want_resid=True, 
     coeffs, csig, resid, info = _alloc_outputs(N, lib.R, Y.device, want_sigma, want_resid, want_info, out)
     with torch.cuda.device(Y.device):
         o = _make_opts(stream=torch.cuda.current_stream().cuda_stream, ldY=ldY,
-                       sigma_pixel_stride=_sigma_stride(sigma, N, lib.L), constraint=constraint,
-                       weighting=weighting, max_iter=max_iter, gap_tol=gap_tol, feas_tol=feas_tol,
+                       sigma_pixel_stride=_sigma_stride(sigma, N, lib.L), constraint=lib.constraint,
+                       weighting=lib.weighting, max_iter=max_iter, gap_tol=gap_tol, feas_tol=feas_tol,
                        info_ptr=None if info is None else info.data_ptr())
         yp = ctypes.c_void_p(Y.data_ptr()) if N > 0 else None
         st = _check(load().linmin_unmix_lib(lib._h, yp, _dev_ptr(sigma, "sigma"), N, ctypes.byref(o),
@@ -277,8 +297,9 @@ def unmix_lib(lib: Library, Y, sigma=None, *, want_sigma=True, want_resid=True, 
 
 
 def unmix(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=True,
-          out: Optional[dict] = None, max_iter=0, gap_tol=0.0, feas_tol=0.0, constraint=0, weighting=0):
-    """linmin_unmix (one-shot: precompute + solve).  All tensors CUDA float32."""
+          out: Optional[dict] = None, max_iter=0, gap_tol=0.0, feas_tol=0.0, constraint=0, cov=None):
+    """linmin_unmix (one-shot: precompute + solve).  All tensors CUDA float32.
+    constraint: CONSTRAINT_*; cov: None | (L,) noise std | (L, L) covariance (renormalised problem, eq. 5-6)."""
     torch = _torch()
     if A.dim() != 2:
         raise ValueError("A must be (L, R)")
@@ -290,11 +311,12 @@ def unmix(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=True,
     _check_tensor(Y, "Y", (N, L), torch.float32, True, A.device)
     _check_sigma(sigma, N, L, True, A.device)
     coeffs, csig, resid, info = _alloc_outputs(N, R, A.device, want_sigma, want_resid, want_info, out)
+    weighting, cov_ptr = _weighting_of(cov, L, True, A.device)
     with torch.cuda.device(A.device):
         o = _make_opts(stream=torch.cuda.current_stream().cuda_stream, ldY=0,
                        sigma_pixel_stride=_sigma_stride(sigma, N, L), constraint=constraint,
                        weighting=weighting, max_iter=max_iter, gap_tol=gap_tol, feas_tol=feas_tol,
-                       info_ptr=None if info is None else info.data_ptr())
+                       info_ptr=None if info is None else info.data_ptr(), cov_ptr=cov_ptr)
         st = _check(load().linmin_unmix(_dev_ptr(A, "A"), _dev_ptr(Y, "Y") if N > 0 else None,
                                         _dev_ptr(sigma, "sigma"), N, L, R, ctypes.byref(o),
                                         _dev_ptr(coeffs, "coeffs"), _dev_ptr(csig, "coeff_sigma"),
@@ -303,7 +325,7 @@ def unmix(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=True,
 
 
 def unmix_host(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=False,
-               out: Optional[dict] = None, max_iter=0, gap_tol=0.0, feas_tol=0.0):
+               out: Optional[dict] = None, max_iter=0, gap_tol=0.0, feas_tol=0.0, constraint=0, cov=None):
     """linmin_unmix_host: numpy arrays or CPU tensors (pinned memory gives full copy bandwidth).
     Blocks until the outputs are complete.  Returns (coeffs, coeff_sigma, resid, info, status) as
     CPU tensors (pinned when freshly allocated)."""
@@ -317,7 +339,7 @@ def unmix_host(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=
             raise ValueError(f"{name} must be a contiguous CPU float32 array")
         return t
 
-    A, Y, sigma = as_cpu(A, "A"), as_cpu(Y, "Y"), as_cpu(sigma, "sigma")
+    A, Y, sigma, cov = as_cpu(A, "A"), as_cpu(Y, "Y"), as_cpu(sigma, "sigma"), as_cpu(cov, "cov")
     if A.dim() != 2:
         raise ValueError("A must be (L, R)")
     L, R = int(A.shape[0]), int(A.shape[1])
@@ -342,7 +364,9 @@ def unmix_host(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=
     if info is None and want_info:
         info = host_empty((N,), torch.int32)
     _check_outputs(N, R, coeffs, csig, resid, info, False)
-    o = _make_opts(ldY=0, sigma_pixel_stride=_sigma_stride(sigma, N, L), max_iter=max_iter,
+    weighting, cov_ptr = _weighting_of(cov, L, False)
+    o = _make_opts(ldY=0, sigma_pixel_stride=_sigma_stride(sigma, N, L), max_iter=max_iter, constraint=constraint,
+                   weighting=weighting, cov_ptr=cov_ptr,
                    gap_tol=gap_tol, feas_tol=feas_tol, info_ptr=None if info is None else info.data_ptr())
 
     def hp(t):

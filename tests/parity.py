@@ -127,3 +127,72 @@ def check_parity(A, Y, sigma, gpu, ora, label="", min_unique=0.99, max_tie_frac=
         pos = ora.coeff_sigma[m] > 1e-6
         stats["max_rel_sigma"] = float((np.abs(sg[m] - ora.coeff_sigma[m])[pos] / ora.coeff_sigma[m][pos]).max()) if pos.any() else 0.0
     return stats
+
+
+def check_parity_next(A, Y, gpu, ora, constraint="sto", cov=None, label="", max_tie_frac=0.005):
+    """Same tolerances for the NEXT-row options: constraint "sto" | "slo" | "pos", and the renormalised
+    problem (cov = (L,) noise std or (L, L) covariance; objective and residual in the C^-1 metric, unit noise for the
+    uncertainties).  The oracle's answer is first certified in numpy (optimality conditions in that metric)."""
+    A64 = A.astype(np.float64); Y64 = Y.astype(np.float64)
+    N, L = Y.shape
+    R = A.shape[1]
+    if cov is None:
+        Ci = np.eye(L)
+    elif cov.ndim == 1:
+        Ci = np.diag(1.0 / cov.astype(np.float64) ** 2)
+    else:
+        Ci = np.linalg.inv(cov.astype(np.float64))
+    a = gpu["coeffs"].astype(np.float64)
+    ao = ora.coeffs
+    assert np.isfinite(a).all(), label
+    # ---- the oracle's optimality in numpy, every pixel
+    g = ((ao @ A64.T - Y64) @ Ci) @ A64
+    F = ao > 0
+    scale = np.abs(g).max(1) + 1e-4 * (np.abs(Y64 @ Ci) @ np.abs(A64)).max(1)
+    if constraint == "sto":
+        nu = -(g * ao).sum(1)
+        assert np.abs(ao.sum(1) - 1).max() <= 1e-12
+    elif constraint == "slo":
+        s = ao.sum(1)
+        nu = np.where(s >= 1 - 1e-12, -(g * ao).sum(1) / np.maximum(s, 1e-300), 0.0)
+        assert s.max() <= 1 + 1e-12 and (nu / scale).min() >= -1e-9, (label, "oracle slo multiplier")
+    else:
+        nu = np.zeros(N)
+    gn = g + nu[:, None]
+    assert (np.abs(np.where(F, gn, 0.0)).max(1) / scale).max() <= 1e-9, (label, "oracle stationarity")
+    assert (np.where(F, 0.0, gn).min(1) / scale).min() >= -1e-9, (label, "oracle multipliers")
+    # ---- feasibility of the GPU answer
+    assert a.min() >= -1e-6, (label, a.min())
+    if constraint == "sto":
+        assert np.abs(a.sum(1) - 1.0).max() <= 1e-5, (label, np.abs(a.sum(1) - 1.0).max())
+    elif constraint == "slo":
+        assert a.sum(1).max() <= 1.0 + 1e-5, (label, a.sum(1).max())
+    # ---- objective in the C^-1 metric (R12)
+    rg = Y64 - a @ A64.T; ro = Y64 - ao @ A64.T
+    Fg = np.einsum("pl,lm,pm->p", rg, Ci, rg); Fo = np.einsum("pl,lm,pm->p", ro, Ci, ro)
+    floor = 1e-12 * np.einsum("pl,lm,pm->p", Y64, Ci, Y64)
+    rel = np.abs(Fg - Fo) / np.maximum(Fo, floor)
+    assert rel.max() <= 1e-5, (label, "objective", rel.max(), int(rel.argmax()))
+    sing = np.linalg.svd(A64, compute_uv=False)
+    unique = ora.rank_margin > 1e-6 * sing[0] * (np.sqrt(np.linalg.eigvalsh(Ci).min()) if cov is not None else 1.0)
+    assert unique.mean() >= 0.99, (label, "unique fraction", unique.mean())
+    da = np.abs(a - ao).max(1)
+    assert da[unique].max() <= 1e-4, (label, "coeffs", da[unique].max(), int(np.argmax(np.where(unique, da, 0))))
+    stats = dict(pixels=int(N), max_da=float(da[unique].max()), max_rel_obj=float(rel.max()))
+    if gpu.get("resid") is not None:
+        rr = np.abs(gpu["resid"].astype(np.float64) - ora.resid) / np.maximum(ora.resid, np.sqrt(floor / L))
+        assert rr.max() <= 1e-5, (label, "resid", rr.max())
+        stats["max_rel_resid"] = float(rr.max())
+    if gpu.get("coeff_sigma") is not None:
+        sg = gpu["coeff_sigma"].astype(np.float64)
+        same = ((a > 0) == (ao > 0)).all(1)
+        err = np.abs(sg - ora.coeff_sigma) - (0.01 * ora.coeff_sigma + 1e-7)
+        m = same & unique
+        assert err[m].max() <= 0, (label, "sigma", err[m].max())
+        ties = np.nonzero(~same & unique)[0]
+        assert len(ties) <= max(2, max_tie_frac * N), (label, "support mismatches", len(ties))
+        for p in ties:
+            diff = (a[p] > 0) ^ (ao[p] > 0)
+            assert max(a[p][diff].max(), ao[p][diff].max()) < 1e-4, (label, p)
+        stats["n_support_ties"] = int(len(ties))
+    return stats

@@ -34,15 +34,16 @@ def test_exports_match_header(lib):
 def test_version_and_strerror(lib):
     from paper_1402_2518_b200 import linmin
     assert linmin.version() == 200
-    for code in [0, -1, -2, -3, -4, -5, -6, 1]:
+    for code in [0, -1, -2, -3, -4, -5, -6, -7, 1]:
         assert "unknown" not in linmin.strerror(code)
     assert "unknown" in linmin.strerror(12345)
 
 
 def test_opts_struct_layout(lib):
     from paper_1402_2518_b200 import linmin
-    # must match include/linmin.h: 4+pad4, 8, 8, 8, 4, 4, 4, 4, 4 +pad4, 8, 4, 4 = 72 bytes
-    assert ctypes.sizeof(linmin.LinminOpts) == 72
+    # must match include/linmin.h: 4+pad4, 8, 8, 8, 4, 4, 4, 4, 4 +pad4, 8, 4, 4, 8 = 80 bytes
+    assert ctypes.sizeof(linmin.LinminOpts) == 80
+    assert linmin.LinminOpts.cov.offset == 72
     assert linmin.LinminOpts.info_out.offset == 56
 
 
@@ -62,8 +63,9 @@ def test_argument_validation_without_device(lib):
     bad = linmin._make_opts(); bad.struct_size = 8
     assert f(one, one, None, 1, 4, 2, ctypes.byref(bad), one, None, None) == linmin.ERR_INVALID_ARGUMENT
     for kw, code in [(dict(ldY=3), -1), (dict(sigma_pixel_stride=2), -1), (dict(max_iter=256), -1),
-                     (dict(gap_tol=-1.0), -1), (dict(constraint=1), -3), (dict(constraint=2), -3),
-                     (dict(constraint=7), -1), (dict(weighting=1), -3), (dict(weighting=9), -1)]:
+                     (dict(gap_tol=-1.0), -1), (dict(constraint=7), -1), (dict(constraint=-1), -1),
+                     (dict(weighting=1), -1), (dict(weighting=2), -1),       # a weighting without opts->cov
+                     (dict(weighting=9), -1)]:
         ob = linmin._make_opts(**kw)
         assert f(one, one, None, 1, 4, 2, ctypes.byref(ob), one, None, None) == code, kw
     h = ctypes.c_void_p()

@@ -1,0 +1,111 @@
+"""-m gpu: the NEXT rows of SURVEY.md 8(f) through the C ABI against the fp64 oracle on the same seeded inputs:
+constraint variants slo / pos and the renormalised problem (eq. 5-6).
+Tolerances: tests/parity.py::check_parity_next (north_star's)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def lm():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1402_2518_b200 import build, linmin
+    build.build_library()
+    linmin.load()
+    return linmin
+
+
+def run_gpu(lm, A, Y, sigma=None, constraint=0, cov=None):
+    dev = torch.device("cuda:0")
+    t = lambda x: None if x is None else torch.from_numpy(np.ascontiguousarray(x)).to(dev)
+    c, s, r, info, status = lm.unmix(t(A), t(Y), t(sigma), constraint=constraint, cov=t(cov))
+    torch.cuda.synchronize()
+    return dict(coeffs=c.cpu().numpy(), coeff_sigma=s.cpu().numpy(), resid=r.cpu().numpy(), info=info.cpu().numpy(), status=status)
+
+
+def shaded(w, seed):
+    """The workload's spectra times a per-pixel brightness factor in [0.5, 1.15] (shade / illumination: the case the
+    sum-lower-than-one option is made for): the coefficients then sum to less or more than one."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    f = rng.uniform(0.5, 1.15, size=(w.N, 1)).astype(np.float32)
+    return (w.Y * f).astype(np.float32)
+
+
+def banded_cov(L, seed, smin=0.002, smax=0.01, rho=0.6, band=3):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    s = rng.uniform(smin, smax, L)
+    idx = np.arange(L)
+    C = (rho ** np.abs(idx[:, None] - idx[None, :])) * np.outer(s, s)
+    C[np.abs(idx[:, None] - idx[None, :]) > band] = 0.0
+    C += 0.05 * np.diag(s ** 2)
+    return C.astype(np.float32)
+
+
+@pytest.mark.parametrize("name,N", [("tiny", 1000), ("omega", 8192), ("crism", 2048)])
+@pytest.mark.parametrize("constraint", ["slo", "pos"])
+def test_constraint_variants(lm, name, N, constraint):
+    import oracle
+    from paper_1402_2518_b200.synth import make_workload
+    from parity import check_parity_next
+    w = make_workload(name, N=N)
+    Y = shaded(w, 11)
+    code = dict(slo=lm.CONSTRAINT_SUM_LOWER_THAN_ONE, pos=lm.CONSTRAINT_POSITIVITY_ONLY)[constraint]
+    g = run_gpu(lm, w.A, Y, w.sigma, constraint=code)
+    ora = oracle.solve(w.A, Y, w.sigma, constraint=constraint)
+    stats = check_parity_next(w.A, Y, g, ora, constraint=constraint, label=f"{name}/{constraint}")
+    s = g["coeffs"].sum(1)
+    assert (s < 0.99).mean() > 0.2                 # the option matters on this input
+    if constraint == "slo":
+        assert (s > 1 - 1e-5).mean() > 0.05        # ... and the bound is active on part of it
+    assert (((g["coeffs"] > 0).sum(1)) == ((g["info"] >> 24) & 0xff)).all()
+    print(name, constraint, stats)
+
+
+@pytest.mark.parametrize("name,N", [("tiny", 1000), ("omega", 8192), ("crism", 2048)])
+@pytest.mark.parametrize("kind", ["diag", "full"])
+def test_renormalised_problem(lm, name, N, kind):
+    """Noise drawn from ONE covariance for the whole cube, fitted with that covariance."""
+    import oracle
+    from paper_1402_2518_b200.synth import make_workload
+    from parity import check_parity_next
+    w = make_workload(name, N=N)
+    C = banded_cov(w.L, 5, band=0 if kind == "diag" else 3)
+    rng = np.random.Generator(np.random.PCG64(17))
+    clean = w.a0 @ w.A.astype(np.float64).T
+    Y = (clean + rng.multivariate_normal(np.zeros(w.L), C.astype(np.float64), size=w.N)).astype(np.float32)
+    cov = np.sqrt(np.diag(C)).astype(np.float32) if kind == "diag" else C
+    g = run_gpu(lm, w.A, Y, None, cov=cov)
+    ora = oracle.solve(w.A, Y, cov=cov)
+    stats = check_parity_next(w.A, Y, g, ora, cov=cov, label=f"{name}/{kind}")
+    # whitened RMS is about 1 when the model fits to the noise (reading R17)
+    assert 0.8 < np.median(g["resid"]) < 1.1
+    print(name, kind, stats)
+
+
+def test_renormalised_slo_and_handle_and_errors(lm):
+    """The OMEGA run of the paper: renormalised AND sum-lower-than-one; handle form; option checks."""
+    import oracle
+    from paper_1402_2518_b200.synth import make_workload
+    from parity import check_parity_next
+    w = make_workload("omega", N=4096)
+    C = banded_cov(w.L, 7)
+    Y = shaded(w, 3)
+    dev = torch.device("cuda:0")
+    lib = lm.library_create(torch.from_numpy(w.A).to(dev), constraint=lm.CONSTRAINT_SUM_LOWER_THAN_ONE, cov=torch.from_numpy(C).to(dev))
+    c, s, r, info, st = lm.unmix_lib(lib, torch.from_numpy(Y).to(dev), None)
+    torch.cuda.synchronize()
+    ora = oracle.solve(w.A, Y, constraint="slo", cov=C)
+    g = dict(coeffs=c.cpu().numpy(), coeff_sigma=s.cpu().numpy(), resid=r.cpu().numpy())
+    print(check_parity_next(w.A, Y, g, ora, constraint="slo", cov=C, label="omega/slo+cov"))
+    # host entry point, same options: identical bits
+    ch, sh, rh, _, _ = lm.unmix_host(w.A, Y, None, constraint=lm.CONSTRAINT_SUM_LOWER_THAN_ONE, cov=C)
+    assert np.array_equal(ch.numpy(), g["coeffs"]) and np.array_equal(sh.numpy(), g["coeff_sigma"]) and np.array_equal(rh.numpy(), g["resid"])
+    lib.destroy()
+    # a covariance that is not positive definite is refused
+    with pytest.raises(lm.LinminError) as e:
+        lm.library_create(torch.from_numpy(w.A).to(dev), cov=torch.from_numpy(-np.eye(w.L, dtype=np.float32)).to(dev))
+    assert e.value.code == lm.ERR_COVARIANCE
