@@ -176,6 +176,44 @@ int linmin_library_last_timing(const linmin_library *lib, float *ipls_ms, float 
  * what is not in use to the driver (call it when idle; the next call allocates again).  Thread-safe. */
 int linmin_trim_memory(void);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * NEXT rows 3-4 of SURVEY.md 8(f): library builder, detection layer, autofit.  Device pointers; `stream` is a
+ * cudaStream_t (NULL = default stream); all enqueue and return unless stated otherwise.
+ */
+
+/* The paper's additional spectra: n_extra = 4 -> Flat 1, Flat 0.0001, Slope increasing,
+ * Slope decreasing; n_extra = 12 -> also cos, sin, -cos, -sin over a quarter period and over half a period of the
+ * spectral domain (reading R18).  Written as columns col0 .. col0 + n_extra - 1 of the L x ld_out
+ * row-major library `out`; wavelength: L increasing values (position = normalised wavelength) or NULL (position =
+ * l / (L - 1)). */
+int linmin_additional_spectra(const float *wavelength, int32_t L, int32_t n_extra, float *out, int32_t ld_out,
+                              int32_t col0, void *stream);
+
+/* Detection threshold per endmember, eq. 8, from a LABELLED set: coeffs N x R estimated
+ * coefficients, present N x R bytes (non-zero: the endmember is part of the true mixture).  A+ / A- are the
+ * detections (coefficient > 0) on present / absent pixels; population std; an empty class contributes 0 (R19).
+ * thresholds_out: R floats.  Sums in fp64 in a fixed order (results do not depend on scheduling). */
+int linmin_detection_thresholds(const float *coeffs, const unsigned char *present, int64_t N, int32_t R,
+                                float *thresholds_out, void *stream);
+
+/* The three detection conditions of PAPER.md:239-246: mask[p*R + i] = coeffs > thresholds[i] and coeff_sigma < coeffs
+ * and resid[p] < rms_max ("10 times the dark current noise").  counts_out (optional): R detections per endmember. */
+int linmin_detect(const float *coeffs, const float *coeff_sigma, const float *resid, const float *thresholds,
+                  float rms_max, int64_t N, int32_t R, unsigned char *mask_out, unsigned long long *counts_out,
+                  void *stream);
+
+/* Second pass "with the detected spectrum only": linmin_unmix against the columns of A whose byte in
+ * keep (R bytes, device) is non-zero; coefficients and uncertainties of the other endmembers are 0.  SYNCHRONISES
+ * opts->stream once (the size of the sub-library decides the allocations). */
+int linmin_second_pass(const float *A, const float *Y, const float *sigma, int64_t N, int32_t L, int32_t R,
+                       const unsigned char *keep, const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out,
+                       float *resid_out);
+
+/* "Autofit" degeneracy test of a library (eq. 7): for every endmember n the residue E of its best
+ * fit by all the OTHER endmembers, unconstrained (resid_ls_out, L x R, column n) and under positivity
+ * (resid_nn_out, L x R; the pos option of the solver).  Either output may be NULL. */
+int linmin_autofit(const float *A, int32_t L, int32_t R, void *stream, float *resid_ls_out, float *resid_nn_out);
+
 const char *linmin_strerror(int code);
 int linmin_version(void);
 

@@ -19,6 +19,7 @@
 #include "ipls_q32.cuh"
 #include "precompute.cuh"
 #include "whiten.cuh"
+#include "detect.cuh"
 
 using namespace linmin;
 
@@ -613,6 +614,151 @@ int linmin_unmix_host(const float *A, const float *Y, const float *sigma, int64_
     cleanup();
     return wrc;
 #undef CKH
+}
+
+// ---------------------------------------------------------------- NEXT rows 3-4: detect.cuh
+
+int linmin_additional_spectra(const float *wavelength, int32_t L, int32_t n_extra, float *out, int32_t ld_out,
+                              int32_t col0, void *stream) {
+    if (!out || L < 1 || (n_extra != 4 && n_extra != 12) || col0 < 0 || ld_out < col0 + n_extra) return LINMIN_ERR_INVALID_ARGUMENT;
+    if (L > LINMIN_MAX_L) return LINMIN_ERR_UNSUPPORTED_SIZE;
+    additional_spectra_kernel<<<(L + 127) / 128, 128, 0, (cudaStream_t)stream>>>(wavelength, L, n_extra, out, ld_out, col0);
+    CK(cudaGetLastError());
+    return LINMIN_OK;
+}
+
+int linmin_detection_thresholds(const float *coeffs, const unsigned char *present, int64_t N, int32_t R,
+                                float *thresholds_out, void *stream) {
+    if (!coeffs || !present || !thresholds_out || N < 0 || R < 1) return LINMIN_ERR_INVALID_ARGUMENT;
+    if (R > LINMIN_MAX_R) return LINMIN_ERR_UNSUPPORTED_SIZE;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int block = R * std::max(1, 256 / R);
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N * R + block - 1) / block, (int64_t)sms * 8));
+    double *part = nullptr;
+    CK(staging_alloc((void **)&part, (size_t)grid * R * 6 * sizeof(double), st));
+    threshold_partial_kernel<<<grid, block, (size_t)block * 6 * sizeof(double), st>>>(coeffs, present, N, R, part);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) {
+        threshold_final_kernel<<<(R + 63) / 64, 64, 0, st>>>(part, grid, R, thresholds_out);
+        e = cudaGetLastError();
+    }
+    cudaFreeAsync(part, st);
+    CK(e);
+    return LINMIN_OK;
+}
+
+int linmin_detect(const float *coeffs, const float *coeff_sigma, const float *resid, const float *thresholds,
+                  float rms_max, int64_t N, int32_t R, unsigned char *mask_out, unsigned long long *counts_out, void *stream) {
+    if (!coeffs || !coeff_sigma || !resid || !thresholds || !mask_out || N < 0 || R < 1) return LINMIN_ERR_INVALID_ARGUMENT;
+    if (R > LINMIN_MAX_R) return LINMIN_ERR_UNSUPPORTED_SIZE;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (counts_out) CK(cudaMemsetAsync(counts_out, 0, (size_t)R * sizeof(unsigned long long), st));
+    if (N == 0) return LINMIN_OK;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N * R + 255) / 256, (int64_t)sms * 8));
+    detect_kernel<<<grid, 256, (size_t)R * sizeof(unsigned int), st>>>(coeffs, coeff_sigma, resid, thresholds, rms_max, N, R,
+                                                                        mask_out, counts_out);
+    CK(cudaGetLastError());
+    return LINMIN_OK;
+}
+
+int linmin_second_pass(const float *A, const float *Y, const float *sigma, int64_t N, int32_t L, int32_t R,
+                       const unsigned char *keep, const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out,
+                       float *resid_out) {
+    int rc = check_sizes(N, L, R);
+    if (rc != LINMIN_OK) return rc;
+    if (!A || !keep || (N > 0 && (!Y || !coeffs_out))) return LINMIN_ERR_INVALID_ARGUMENT;
+    Resolved o;
+    rc = resolve_opts(opts, L, &o);
+    if (rc != LINMIN_OK) return rc;
+    // the size of the sub-library decides every allocation below: the one place where the host reads device data
+    std::vector<unsigned char> hk((size_t)R);
+    CK(cudaMemcpyAsync(hk.data(), keep, (size_t)R, cudaMemcpyDeviceToHost, o.stream));
+    CK(cudaStreamSynchronize(o.stream));
+    std::vector<int> idx;
+    for (int i = 0; i < R; ++i) if (hk[i]) idx.push_back(i);
+    const int Rs = (int)idx.size();
+    if (Rs < 1) return LINMIN_ERR_INVALID_ARGUMENT;
+    int *didx = nullptr;
+    float *sub = nullptr, *cs = nullptr, *ss = nullptr;
+    struct FreeV { void *p; cudaStream_t s; ~FreeV() { if (p) cudaFreeAsync(p, s); } };
+    CK(staging_alloc((void **)&didx, (size_t)Rs * sizeof(int), o.stream));
+    FreeV f0{didx, o.stream};
+    CK(cudaMemcpyAsync(didx, idx.data(), (size_t)Rs * sizeof(int), cudaMemcpyHostToDevice, o.stream));
+    CK(cudaStreamSynchronize(o.stream));     // idx is a host vector that dies with this call
+    CK(staging_alloc((void **)&sub, (size_t)L * Rs * sizeof(float), o.stream));
+    FreeV f1{sub, o.stream};
+    gather_columns_kernel<<<(L * Rs + 255) / 256, 256, 0, o.stream>>>(A, L, R, didx, Rs, sub);
+    CK(cudaGetLastError());
+    if (N == 0) return LINMIN_OK;
+    CK(staging_alloc((void **)&cs, (size_t)N * Rs * sizeof(float), o.stream));
+    FreeV f2{cs, o.stream};
+    if (coeff_sigma_out) CK(staging_alloc((void **)&ss, (size_t)N * Rs * sizeof(float), o.stream));
+    FreeV f3{ss, o.stream};
+    rc = linmin_unmix(sub, Y, sigma, N, L, Rs, opts, cs, ss, resid_out);
+    if (rc < 0) return rc;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N * Rs + 255) / 256, (int64_t)sms * 8));
+    CK(cudaMemsetAsync(coeffs_out, 0, (size_t)N * R * sizeof(float), o.stream));
+    scatter_columns_kernel<<<grid, 256, 0, o.stream>>>(cs, N, Rs, didx, R, coeffs_out);
+    CK(cudaGetLastError());
+    if (coeff_sigma_out) {
+        CK(cudaMemsetAsync(coeff_sigma_out, 0, (size_t)N * R * sizeof(float), o.stream));
+        scatter_columns_kernel<<<grid, 256, 0, o.stream>>>(ss, N, Rs, didx, R, coeff_sigma_out);
+        CK(cudaGetLastError());
+    }
+    return rc;
+}
+
+int linmin_autofit(const float *A, int32_t L, int32_t R, void *stream, float *resid_ls_out, float *resid_nn_out) {
+    int rc = check_sizes(0, L, R);
+    if (rc != LINMIN_OK) return rc;
+    if (!A || R < 2 || (!resid_ls_out && !resid_nn_out)) return LINMIN_ERR_INVALID_ARGUMENT;
+    cudaStream_t st = (cudaStream_t)stream;
+    struct FreeV { void *p; cudaStream_t s; ~FreeV() { if (p) cudaFreeAsync(p, s); } };
+    if (resid_ls_out) {
+        double *Q = nullptr;
+        CK(staging_alloc((void **)&Q, (size_t)R * L * (R - 1) * sizeof(double), st));
+        FreeV fq{Q, st};
+        autofit_ls_kernel<<<R, 256, 0, st>>>(A, L, R, Q, resid_ls_out);
+        CK(cudaGetLastError());
+    }
+    if (resid_nn_out) {
+        // eq. 7 under positivity: R problems of R - 1 endmembers through the pos option of the solver (N = 1 each)
+        float *Sn = nullptr, *yrow = nullptr, *a = nullptr;
+        CK(staging_alloc((void **)&Sn, (size_t)L * (R - 1) * sizeof(float), st));
+        FreeV f0{Sn, st};
+        CK(staging_alloc((void **)&yrow, (size_t)L * sizeof(float), st));
+        FreeV f1{yrow, st};
+        CK(staging_alloc((void **)&a, (size_t)(R - 1) * sizeof(float), st));
+        FreeV f2{a, st};
+        Resolved o;
+        resolve_opts(nullptr, L, &o);
+        o.stream = st; o.constraint = LINMIN_CONSTRAINT_POSITIVITY_ONLY;
+        for (int n = 0; n < R; ++n) {
+            drop_column_kernel<<<(L * (R - 1) + 255) / 256, 256, 0, st>>>(A, L, R, n, Sn, yrow);
+            CK(cudaGetLastError());
+            linmin_library *lib = nullptr;
+            int wrc = library_create_impl(Sn, L, R - 1, st, false, false, LINMIN_CONSTRAINT_POSITIVITY_ONLY,
+                                          LINMIN_WEIGHTING_NONE, nullptr, &lib);
+            if (wrc < 0) return wrc;
+            rc = launch_solve(lib, yrow, nullptr, 1, o, a, nullptr, nullptr);
+            if (rc == LINMIN_OK) {
+                autofit_residue_kernel<<<(L + 127) / 128, 128, 0, st>>>(A, L, R, n, Sn, a, resid_nn_out);
+                if (cudaGetLastError() != cudaSuccess) rc = LINMIN_ERR_CUDA;
+            }
+            linmin_library_destroy(lib);
+            if (rc != LINMIN_OK) return rc;
+        }
+    }
+    return LINMIN_OK;
 }
 
 }  // extern "C"

@@ -37,7 +37,9 @@ INFO_LIBRARY_NONFINITE = 0x40
 EXPORTS = ["linmin_version", "linmin_strerror", "linmin_library_create", "linmin_library_destroy",
            "linmin_library_last_launches", "linmin_library_enable_timing", "linmin_library_last_timing",
            "linmin_trim_memory",
-           "linmin_unmix_lib", "linmin_unmix", "linmin_unmix_host"]
+           "linmin_unmix_lib", "linmin_unmix", "linmin_unmix_host",
+           "linmin_additional_spectra", "linmin_detection_thresholds", "linmin_detect", "linmin_second_pass",
+           "linmin_autofit"]
 
 
 class LinminOpts(ctypes.Structure):
@@ -79,6 +81,11 @@ def load() -> ctypes.CDLL:
         lib.linmin_unmix_lib.argtypes = [P, P, P, I64, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_unmix.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_unmix_host.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
+        lib.linmin_additional_spectra.argtypes = [P, I32, I32, P, I32, I32, P]
+        lib.linmin_detection_thresholds.argtypes = [P, P, I64, I32, P, P]
+        lib.linmin_detect.argtypes = [P, P, P, P, ctypes.c_float, I64, I32, P, P, P]
+        lib.linmin_second_pass.argtypes = [P, P, P, I64, I32, I32, P, ctypes.POINTER(LinminOpts), P, P, P]
+        lib.linmin_autofit.argtypes = [P, I32, I32, P, P, P]
         _lib = lib
     return _lib
 
@@ -375,3 +382,95 @@ def unmix_host(A, Y, sigma=None, *, want_sigma=True, want_resid=True, want_info=
     st = _check(load().linmin_unmix_host(hp(A), hp(Y) if N > 0 else None, hp(sigma), N, L, R,
                                          ctypes.byref(o), hp(coeffs), hp(csig), hp(resid)))
     return coeffs, csig, resid, info, st
+
+
+# ------------------------------------------------------------------ NEXT rows 3-4: library builder, detection, autofit
+def _stream():
+    return ctypes.c_void_p(_torch().cuda.current_stream().cuda_stream)
+
+
+def additional_spectra(L, n_extra, device, wavelength=None, out=None, col0=0):
+    """linmin_additional_spectra: (L, n_extra) tensor, or columns col0.. of `out` (L, ld)."""
+    torch = _torch()
+    if out is None:
+        out = torch.empty((L, n_extra), dtype=torch.float32, device=device)
+        col0 = 0
+    _check_tensor(out, "out", (L, out.shape[1]), torch.float32, True)
+    _check_tensor(wavelength, "wavelength", (L,), torch.float32, True, out.device)
+    with torch.cuda.device(out.device):
+        _check(load().linmin_additional_spectra(_dev_ptr(wavelength, "wavelength"), L, n_extra, _dev_ptr(out, "out"),
+                                                int(out.shape[1]), col0, _stream()))
+    return out
+
+
+def build_library(A_ref, n_extra, wavelength=None):
+    """The reference spectra (L, R0) followed by the paper's 4 or 12 additional spectra: (L, R0 + n_extra)."""
+    torch = _torch()
+    L, R0 = int(A_ref.shape[0]), int(A_ref.shape[1])
+    out = torch.empty((L, R0 + n_extra), dtype=torch.float32, device=A_ref.device)
+    out[:, :R0] = A_ref
+    return additional_spectra(L, n_extra, A_ref.device, wavelength, out, R0)
+
+
+def detection_thresholds(coeffs, present):
+    """linmin_detection_thresholds (eq. 8): coeffs (N, R) float32, present (N, R) uint8 / bool -> (R,) float32."""
+    torch = _torch()
+    N, R = int(coeffs.shape[0]), int(coeffs.shape[1])
+    present = present.to(torch.uint8)
+    _check_tensor(coeffs, "coeffs", (N, R), torch.float32, True)
+    _check_tensor(present, "present", (N, R), torch.uint8, True, coeffs.device)
+    thr = torch.empty((R,), dtype=torch.float32, device=coeffs.device)
+    with torch.cuda.device(coeffs.device):
+        _check(load().linmin_detection_thresholds(_dev_ptr(coeffs, "coeffs"), ctypes.c_void_p(present.data_ptr()), N, R,
+                                                  _dev_ptr(thr, "thr"), _stream()))
+    return thr
+
+
+def detect(coeffs, coeff_sigma, resid, thresholds, rms_max):
+    """linmin_detect: (mask (N, R) uint8, counts (R,) int64)."""
+    torch = _torch()
+    N, R = int(coeffs.shape[0]), int(coeffs.shape[1])
+    _check_tensor(coeffs, "coeffs", (N, R), torch.float32, True)
+    _check_tensor(coeff_sigma, "coeff_sigma", (N, R), torch.float32, True, coeffs.device)
+    _check_tensor(resid, "resid", (N,), torch.float32, True, coeffs.device)
+    _check_tensor(thresholds, "thresholds", (R,), torch.float32, True, coeffs.device)
+    mask = torch.empty((N, R), dtype=torch.uint8, device=coeffs.device)
+    counts = torch.empty((R,), dtype=torch.int64, device=coeffs.device)
+    with torch.cuda.device(coeffs.device):
+        _check(load().linmin_detect(_dev_ptr(coeffs, "coeffs"), _dev_ptr(coeff_sigma, "coeff_sigma"), _dev_ptr(resid, "resid"),
+                                    _dev_ptr(thresholds, "thresholds"), ctypes.c_float(rms_max), N, R,
+                                    ctypes.c_void_p(mask.data_ptr()), ctypes.c_void_p(counts.data_ptr()), _stream()))
+    return mask, counts
+
+
+def second_pass(A, Y, sigma, keep, *, constraint=0, cov=None):
+    """linmin_second_pass: keep (R,) uint8 / bool.  Returns (coeffs, coeff_sigma, resid, status)."""
+    torch = _torch()
+    L, R = int(A.shape[0]), int(A.shape[1])
+    N = int(Y.shape[0])
+    _check_tensor(A, "A", (L, R), torch.float32, True)
+    _check_tensor(Y, "Y", (N, L), torch.float32, True, A.device)
+    _check_sigma(sigma, N, L, True, A.device)
+    keep = keep.to(torch.uint8)
+    _check_tensor(keep, "keep", (R,), torch.uint8, True, A.device)
+    coeffs, csig, resid, _ = _alloc_outputs(N, R, A.device, True, True, False, None)
+    weighting, cov_ptr = _weighting_of(cov, L, True, A.device)
+    with torch.cuda.device(A.device):
+        o = _make_opts(stream=torch.cuda.current_stream().cuda_stream, sigma_pixel_stride=_sigma_stride(sigma, N, L),
+                       constraint=constraint, weighting=weighting, cov_ptr=cov_ptr)
+        st = _check(load().linmin_second_pass(_dev_ptr(A, "A"), _dev_ptr(Y, "Y"), _dev_ptr(sigma, "sigma"), N, L, R,
+                                              ctypes.c_void_p(keep.data_ptr()), ctypes.byref(o), _dev_ptr(coeffs, "coeffs"),
+                                              _dev_ptr(csig, "coeff_sigma"), _dev_ptr(resid, "resid")))
+    return coeffs, csig, resid, st
+
+
+def autofit(A):
+    """linmin_autofit (eq. 7): (E_ls, E_nn), each (L, R): residues of every endmember against the others."""
+    torch = _torch()
+    L, R = int(A.shape[0]), int(A.shape[1])
+    _check_tensor(A, "A", (L, R), torch.float32, True)
+    E_ls = torch.empty((L, R), dtype=torch.float32, device=A.device)
+    E_nn = torch.empty((L, R), dtype=torch.float32, device=A.device)
+    with torch.cuda.device(A.device):
+        _check(load().linmin_autofit(_dev_ptr(A, "A"), L, R, _stream(), _dev_ptr(E_ls, "E_ls"), _dev_ptr(E_nn, "E_nn")))
+    return E_ls, E_nn

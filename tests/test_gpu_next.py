@@ -109,3 +109,73 @@ def test_renormalised_slo_and_handle_and_errors(lm):
     with pytest.raises(lm.LinminError) as e:
         lm.library_create(torch.from_numpy(w.A).to(dev), cov=torch.from_numpy(-np.eye(w.L, dtype=np.float32)).to(dev))
     assert e.value.code == lm.ERR_COVARIANCE
+
+
+# ------------------------------------------------------------------ NEXT rows 3-4: library builder, detection layer, autofit
+def test_library_builder_detection_layer_and_second_pass(lm):
+    """PAPER.md:112-114, 149-153 (eq. 8), 239-246, 294 against oracle/detect.py on the same arrays."""
+    import oracle
+    from oracle import detect as D
+    from paper_1402_2518_b200.synth import make_workload
+    dev = torch.device("cuda:0")
+    w = make_workload("omega", N=20000)
+    # library builder: 28 reference spectra + the paper's 4 additional spectra, and the 12-spectra set on a wavelength grid
+    wl = torch.from_numpy(w.wavelength.astype(np.float32)).to(dev)
+    lib36 = lm.build_library(torch.from_numpy(w.A[:, :28]).to(dev), 4)
+    assert lib36.shape == (w.L, 32)
+    np.testing.assert_allclose(lib36[:, 28:].cpu().numpy(), D.additional_spectra(w.L, 4), atol=1e-7)
+    e12 = lm.additional_spectra(w.L, 12, dev, wavelength=wl).cpu().numpy()
+    np.testing.assert_allclose(e12, D.additional_spectra(w.L, 12, w.wavelength.astype(np.float32)), atol=2e-7)
+    # thresholds (eq. 8) on the labelled synthetic set, from the GPU's own coefficients
+    A, Y, S = (torch.from_numpy(x).to(dev) for x in (w.A, w.Y, w.sigma))
+    c, s, r, info, _ = lm.unmix(A, Y, S)
+    present = torch.from_numpy(w.a0 > 0).to(dev)
+    thr = lm.detection_thresholds(c, present)
+    cn, sn, rn = c.cpu().numpy(), s.cpu().numpy(), r.cpu().numpy()
+    thr_ref = D.thresholds(cn, w.a0 > 0)
+    np.testing.assert_allclose(thr.cpu().numpy(), thr_ref, rtol=2e-6, atol=1e-9)
+    thr2 = lm.detection_thresholds(c, present)
+    assert torch.equal(thr, thr2)                                   # fixed summation order
+    # detection mask: bit-exact against the definition evaluated on the same float32 arrays
+    rms_max = 0.0065
+    mask, counts = lm.detect(c, s, r, thr, rms_max)
+    mref, cref = D.detect(cn, sn, rn, thr.cpu().numpy(), np.float32(rms_max))
+    assert np.array_equal(mask.cpu().numpy().astype(bool), mref)
+    assert np.array_equal(counts.cpu().numpy(), cref)
+    assert 0 < mref.sum() < mref.size and (rn < rms_max).mean() > 0.3
+    # second pass on the detected endmembers (plus the extra spectra, which are always kept)
+    keep = torch.zeros(w.R, dtype=torch.bool, device=dev)
+    keep[counts.topk(12).indices] = True                    # the twelve most often detected endmembers
+    keep[28:] = True
+    assert 4 < int(keep.sum()) < w.R
+    c2, s2, r2, _ = lm.second_pass(A, Y, S, keep)
+    kn = keep.cpu().numpy()
+    direct = lm.unmix(torch.from_numpy(np.ascontiguousarray(w.A[:, kn])).to(dev), Y, S)
+    torch.cuda.synchronize()
+    assert torch.equal(c2[:, keep], direct[0]) and torch.equal(s2[:, keep], direct[1]) and torch.equal(r2, direct[2])
+    assert float(c2[:, ~keep].abs().max()) == 0.0
+    from parity import check_parity
+    sel = np.arange(0, w.N, 10)
+    oc, osig, ores = D.second_pass(w.A, w.Y[sel], w.sigma[sel], kn, oracle.solve)
+    np.testing.assert_allclose(c2.cpu().numpy()[sel], oc, atol=1e-4)
+    np.testing.assert_allclose(r2.cpu().numpy()[sel], ores, rtol=1e-5)
+
+
+@pytest.mark.parametrize("name", ["tiny", "omega", "crism"])
+def test_autofit(lm, name):
+    """eq. 7: residues of every endmember against the others, unconstrained and under positivity."""
+    import oracle
+    from oracle import detect as D
+    from paper_1402_2518_b200.synth import make_workload
+    w = make_workload(name, N=4)
+    dev = torch.device("cuda:0")
+    E_ls, E_nn = lm.autofit(torch.from_numpy(w.A).to(dev))
+    torch.cuda.synchronize()
+    R_ls, R_nn = D.autofit(w.A, lambda A, Y: oracle.solve(A, Y, constraint="pos"))
+    scale = np.linalg.norm(w.A.astype(np.float64), axis=0)
+    # residues as vectors, relative to the norm of the endmember they are residues of
+    assert (np.linalg.norm(E_nn.cpu().numpy() - R_nn, axis=0) / scale).max() <= 1e-5
+    assert (np.linalg.norm(E_ls.cpu().numpy() - R_ls, axis=0) / scale).max() <= 1e-5
+    n_ls, n_nn = np.linalg.norm(E_ls.cpu().numpy(), axis=0), np.linalg.norm(E_nn.cpu().numpy(), axis=0)
+    assert (n_nn >= n_ls - 1e-6 * scale).all()              # PAPER.md:100: positivity never fits better
+    print(name, "median residue norm / endmember norm: unconstrained %.3g, positivity %.3g" % (np.median(n_ls / scale), np.median(n_nn / scale)))
