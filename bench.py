@@ -169,6 +169,62 @@ def run_reference(args, rank, world):
     }))
 
 
+def time_calls(torch, fn, reps=3):
+    fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def run_extras(linmin, torch, dev, A4, Yd, Sd):
+    """Not the headline: (a) BASELINE.json configs[2] and [3] (R = 64, R = 256: the any-size kernels), whole config,
+    with the per-kernel split and the fraction of the FP32 peak in SURVEY 8(d) flops; (b) the NEXT-row options of
+    SURVEY.md 8(f) on the first 2^20 pixels of the timed workload."""
+    from paper_1402_2518_b200.synth import make_workload
+    out = {"configs": {}, "options": {}}
+    for name in ("crism", "stress"):
+        w = make_workload(name)
+        At, Yt, St = (torch.from_numpy(x).to(dev) for x in (w.A, w.Y, w.sigma))
+        lib = linmin.library_create(At)
+        lib.enable_timing(True)
+        res = {}
+
+        def call():
+            res["o"] = linmin.unmix_lib(lib, Yt, St)
+        ms = time_calls(torch, call, reps=2 if name == "stress" else 3)
+        ipls_ms, fin_ms = lib.last_timing()
+        info = res["o"][3].cpu().numpy()
+        it, piv, k = (info >> 8) & 0xff, (info >> 16) & 0xff, (info >> 24) & 0xff
+        f_ipls, f_fin = flops_model(w.L, w.R, it, piv, k)
+        out["configs"][name] = {"L": w.L, "R": w.R, "N": w.N, "ms": ms, "spectra_per_s": w.N / (ms * 1e-3),
+                                "ipls_ms": ipls_ms, "finish_ms": fin_ms, "mean_iterations": float(it.mean()),
+                                "ipls_frac_of_fp32_peak": f_ipls / (ipls_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
+                                "whole_frac_of_fp32_peak": (f_ipls + f_fin) / (ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS}
+        lib.destroy()
+    n = min(1 << 20, Yd.shape[0])
+    Y1, S1 = Yd[:n], Sd[:n]
+    Ad = torch.from_numpy(A4).to(dev)
+    L = A4.shape[0]
+    sd = Sd[0].clone()
+    idx = torch.arange(L, device=dev)
+    C = (0.6 ** (idx[:, None] - idx[None, :]).abs().float()) * torch.outer(sd, sd)
+    C = torch.where((idx[:, None] - idx[None, :]).abs() > 3, torch.zeros_like(C), C) + 0.05 * torch.diag(sd ** 2)
+    cases = {"sto (headline path)": dict(), "slo": dict(constraint=linmin.CONSTRAINT_SUM_LOWER_THAN_ONE),
+             "pos": dict(constraint=linmin.CONSTRAINT_POSITIVITY_ONLY),
+             "sto + diagonal covariance": dict(cov=sd), "sto + full covariance (banded, 7 diagonals)": dict(cov=C.contiguous())}
+    for label, kw in cases.items():
+        lib = linmin.library_create(Ad, **kw)
+        ms = time_calls(torch, lambda: linmin.unmix_lib(lib, Y1, None if "cov" in kw else S1))
+        out["options"][label] = {"N": n, "ms": ms, "spectra_per_s": n / (ms * 1e-3)}
+        lib.destroy()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -180,6 +236,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--sample", type=int, default=None, help="pixels in the cpu_baseline / reference sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the extra report keys (other configs, NEXT-row options); the headline is unaffected")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -299,7 +357,7 @@ def main():
         ffma_tf, ffma2_tf = None, None
     f_exec = executed_ipls_flops(L, R, it)
     roofline = {
-        "bound": "alu", "kernel": "projection+IPLS kernel (K1)", "achieved": achieved,
+        "bound": "alu", "kernel": "projection + start kernel (K0) and IPLS iteration kernel (K1), timed together", "achieved": achieved,
         "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
         "traffic": traffic,
         "traffic_source": "STORED, not measured by this run: dram bytes per pixel of the ncu --set full capture in "
@@ -349,6 +407,12 @@ def main():
             cpu_baseline = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                             "sample": f"first {n} pixels of the same workload, one pass, {dt:.1f} s"}
 
+    # ---- extra report keys (rank 0, after the timed region): the other BASELINE.json configs through the any-size
+    #      kernels, and the NEXT-row options on the config-4 library -- device-resident, CUDA events, 3 calls each
+    extras = None
+    if rank == 0 and not args.no_extras:
+        extras = run_extras(linmin, torch, dev, A, Yd, Sd)
+
     # ---- end-to-end: host buffers through linmin_unmix_host (H2D + kernels + D2H per step)
     e2e = None
     if args.e2e_steps > 0:
@@ -388,7 +452,7 @@ def main():
             "shared_sigma": {"value": world * N / (ms_shared * 1e-3), "unit": UNIT, "ms_per_step": ms_shared,
                              "what": "same step with ONE shared sigma[L] (sigma_pixel_stride = 0), device-resident"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
-            "cpu_baseline": cpu_baseline, "parity_sample": parity,
+            "cpu_baseline": cpu_baseline, "parity_sample": parity, "extras": extras,
         }
         print(json.dumps(line))
     if world > 1:

@@ -146,6 +146,7 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
 #pragma unroll
     for (int s = 0; s < S; ++s) { a[s] = 1.0f / 32.0f; lam[s] = 1.0f; gmb[s] = 0.0f; }
 
+#pragma unroll 1
     while (true) {
         // ---- residuals and stopping rule (per pixel group)
         float mu, rp;
