@@ -346,8 +346,8 @@ def main():
         try:
             tj = json.load(open(tpath))
             traffic = tj.get("ipls_kernel_dram_bytes_per_pixel", None)
-            if traffic is not None:
-                traffic = traffic * N
+            if traffic is not None:      # K0 and K1 are timed together: both kernels' bytes
+                traffic = (traffic + tj.get("start_r32_kernel_dram_bytes_per_pixel", 0.0)) * N
         except (OSError, ValueError):
             traffic = None
     try:
