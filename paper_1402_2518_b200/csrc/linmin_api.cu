@@ -17,6 +17,7 @@
 #include "finish_fast.cuh"
 #include "ipls_generic.cuh"
 #include "ipls_q32.cuh"
+#include "ipls_w64.cuh"
 #include "precompute.cuh"
 #include "whiten.cuh"
 #include "detect.cuh"
@@ -260,6 +261,10 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
             CK(launch_ipls_q32(lv, prm, pb, pe, recbuf, lib->sm_count, tickets + c, o.stream));
             launches += 2;
         }
+    } else if (cons && R > 32 && R <= 64 && ipls_w64_warps(L) > 0) {
+        // 33..64 endmembers (CRISM-like config, the paper's 36 / 37 / 44 spectra): one warp per pixel, matrix in registers
+        CK(launch_ipls_w64(lv, prm, lib->sm_count, counters, o.stream));
+        ++launches;
     } else if (R <= 64) {
         const int teams = 8, block = teams * 32;
         size_t smem = teams * ipls_warp_team_floats(L, R) * sizeof(float);
