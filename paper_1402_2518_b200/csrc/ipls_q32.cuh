@@ -200,10 +200,12 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
                     const float4 l0 = *reinterpret_cast<const float4 *>(q + 32 + 8 * t), l1 = *reinterpret_cast<const float4 *>(q + 32 + 8 * t + 4);
                     const float4 g0 = *reinterpret_cast<const float4 *>(q + 64 + 8 * t), g1 = *reinterpret_cast<const float4 *>(q + 64 + 8 * t + 4);
                     const float4 sv = *reinterpret_cast<const float4 *>(q + 96);
+                    const float2 mr = *reinterpret_cast<const float2 *>(q + 100);
                     a[0] = a0.x; a[1] = a0.y; a[2] = a0.z; a[3] = a0.w; a[4] = a1.x; a[5] = a1.y; a[6] = a1.z; a[7] = a1.w;
                     lam[0] = l0.x; lam[1] = l0.y; lam[2] = l0.z; lam[3] = l0.w; lam[4] = l1.x; lam[5] = l1.y; lam[6] = l1.z; lam[7] = l1.w;
                     gmb[0] = g0.x; gmb[1] = g0.y; gmb[2] = g0.z; gmb[3] = g0.w; gmb[4] = g1.x; gmb[5] = g1.y; gmb[6] = g1.z; gmb[7] = g1.w;
                     nu = sv.x; sc = sv.y; lam0 = sv.z; flags = __float_as_int(sv.w);
+                    mu = mr.x; rp = mr.y;          // of the start point (K0): no second pass over the residuals
                     iters = 0; pix = np; done = false;
                 } else {
                     idle = true; pix = -1;
@@ -215,7 +217,7 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
             asm volatile("cp.async.commit_group;" ::: "memory");
             head = (head + m) & (QD - 1);
             if (__all_sync(FULL, idle)) break;
-            continue;                     // residuals of the new pixels first
+            // a fresh pixel goes straight into its first Newton step (the stopping rule sees it next time round)
         }
         if (!idle) ++iters;
 

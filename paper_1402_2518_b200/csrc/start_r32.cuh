@@ -13,7 +13,7 @@
 // problem, x = Gi b - q (1'Gi b - 1)/(1'q), its reduced gradient as multipliers, both shifted into the interior.
 // The two 32 x 32 mat-vecs run as packed FMAs over a PAIR of pixels with the matrix row broadcast.
 //
-// Output: one 400-byte record per pixel for the iteration kernel (ipls_q32.cuh): a, lambda, G a - b (each in the
+// Output: one 416-byte record per pixel for the iteration kernel (ipls_q32.cuh): a, lambda, G a - b (each in the
 // lane-major order of that kernel: position 8 t + s holds row t + 4 s), nu, the scale sc, lambda0 and the flags.
 #pragma once
 #include "common.cuh"
@@ -26,7 +26,7 @@ constexpr int WARPS = 8;
 constexpr int TP = 128;        // pixels per warp tile
 constexpr int CH = 16;         // channels per staged chunk
 constexpr int YST = 20;        // padded row stride (floats) of a staged chunk: conflict-free LDS.128 by pixel
-constexpr int REC = 100;       // floats per record: a[32] lambda[32] (Ga - b)[32] nu sc lambda0 flags
+constexpr int REC = 104;       // floats per record: a[32] lambda[32] (Ga - b)[32] nu sc lambda0 flags mu rp - -
 constexpr unsigned FULL = 0xffffffffu;
 
 __host__ __device__ inline int lpad(int L) { return (L + CH - 1) / CH * CH; }
@@ -234,6 +234,7 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
                 if (flat) { lam0 = fmaxf(bmx, 1e-3f * gdmax); nuh = 0.0f; }
                 if (p < p_end) {
                     float *o = rec + (p - p_begin) * REC;
+                    float gap = 0.0f, suma = 0.0f;      // a'lambda and sum a of the start point (mu and r_p of iteration 0)
                     // lane-major order of the iteration kernel: position 8 t + s <- row t + 4 s
 #pragma unroll
                     for (int t = 0; t < 4; ++t)
@@ -248,6 +249,7 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
                                 lv[e] = flat ? lam0 : (gg - bb) + lsh;
                                 // G a of the shifted, normalised point, minus b
                                 gv[e] = (flat ? Grs[r] * (1.0f / 32.0f) : fmaf(xsh, Grs[r], gg) * rsa) - bb;
+                                gap = fmaf(av[e], lv[e], gap); suma += av[e];
                             }
                             *reinterpret_cast<float4 *>(o + 8 * t + 4 * hh) = make_float4(av[0], av[1], av[2], av[3]);
                             *reinterpret_cast<float4 *>(o + 32 + 8 * t + 4 * hh) = make_float4(lv[0], lv[1], lv[2], lv[3]);
@@ -255,6 +257,7 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
                         }
                     const bool bd = h ? bad1 : bad0;
                     *reinterpret_cast<float4 *>(o + 96) = make_float4(nuh, sch, lam0, __int_as_float(bd ? LINMIN_INFO_NONFINITE_INPUT : 0));
+                    *reinterpret_cast<float4 *>(o + 100) = make_float4(gap * (1.0f / 32.0f), suma - 1.0f, 0.0f, 0.0f);
                 }
 #undef H_
             }
