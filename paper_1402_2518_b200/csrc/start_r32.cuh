@@ -158,9 +158,13 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
                 bmax.x = fmaxf(bmax.x, fabsf(b2[r].x)); bmax.y = fmaxf(bmax.y, fabsf(b2[r].y));
             }
             const float2 sc = make_float2(fmaxf(bmax.x, 1e-3f * gdmax), fmaxf(bmax.y, 1e-3f * gdmax));
-            // x = Gi b (matrix rows broadcast from shared memory, packed FMAs over the pixel pair)
-            float2 x2[R];
-#pragma unroll
+            // the pair's slot of the park area is free now: scratch for one vector (x, then G x)
+            float2 *scr = park + pp * R * 32;
+            // x = Gi b (matrix rows broadcast from shared memory, packed FMAs over the pixel pair); the row loop is
+            // ROLLED (the result goes through the scratch vector): straight-line code for both mat-vecs was 50 KB for
+            // 8 warps and the kernel stalled on instruction fetch
+            float2 sx = make_float2(0.0f, 0.0f);
+#pragma unroll 2
             for (int r = 0; r < R; ++r) {
                 float2 s0 = make_float2(0.0f, 0.0f), s1 = make_float2(0.0f, 0.0f);
 #pragma unroll
@@ -169,19 +173,20 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
                     s0 = fma2(g4.x, b2[4 * c4 + 0], s0); s1 = fma2(g4.y, b2[4 * c4 + 1], s1);
                     s0 = fma2(g4.z, b2[4 * c4 + 2], s0); s1 = fma2(g4.w, b2[4 * c4 + 3], s1);
                 }
-                x2[r] = make_float2(s0.x + s1.x, s0.y + s1.y);
+                const float2 xr = make_float2(s0.x + s1.x, s0.y + s1.y);
+                scr[r * 32] = xr;
+                sx.x += xr.x; sx.y += xr.y;
             }
-            float2 sx = make_float2(0.0f, 0.0f);
-#pragma unroll
-            for (int r = 0; r < R; ++r) { sx.x += x2[r].x; sx.y += x2[r].y; }
             const float2 mu0 = make_float2((sx.x - 1.0f) * rGiqTot, (sx.y - 1.0f) * rGiqTot);
+            float2 x2[R];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const float q = Giq[r];
-                x2[r].x = fmaf(-mu0.x, q, x2[r].x); x2[r].y = fmaf(-mu0.y, q, x2[r].y);
+                const float2 xr = scr[r * 32];
+                x2[r] = make_float2(fmaf(-mu0.x, q, xr.x), fmaf(-mu0.y, q, xr.y));
             }
-            // G x
-            float2 ga2[R];
+            // G x into the scratch vector; gradient at x: g = G x - b; nu = -g'x; shifts into the interior
+            float2 gx = make_float2(0.0f, 0.0f), mnx = make_float2(INFINITY, INFINITY), mng = mnx;
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 float2 s0 = make_float2(0.0f, 0.0f), s1 = make_float2(0.0f, 0.0f);
@@ -191,13 +196,9 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
                     s0 = fma2(g4.x, x2[4 * c4 + 0], s0); s1 = fma2(g4.y, x2[4 * c4 + 1], s1);
                     s0 = fma2(g4.z, x2[4 * c4 + 2], s0); s1 = fma2(g4.w, x2[4 * c4 + 3], s1);
                 }
-                ga2[r] = make_float2(s0.x + s1.x, s0.y + s1.y);
-            }
-            // gradient at x: g = G x - b (kept implicit); nu = -g'x; shifts into the interior
-            float2 gx = make_float2(0.0f, 0.0f), mnx = make_float2(INFINITY, INFINITY), mng = mnx;
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const float2 g = make_float2(ga2[r].x - b2[r].x, ga2[r].y - b2[r].y);
+                const float2 gar = make_float2(s0.x + s1.x, s0.y + s1.y);
+                scr[r * 32] = gar;
+                const float2 g = make_float2(gar.x - b2[r].x, gar.y - b2[r].y);
                 gx.x = fmaf(g.x, x2[r].x, gx.x); gx.y = fmaf(g.y, x2[r].y, gx.y);
                 mnx.x = fminf(mnx.x, x2[r].x); mnx.y = fminf(mnx.y, x2[r].y);
                 mng.x = fminf(mng.x, g.x); mng.y = fminf(mng.y, g.y);
@@ -210,7 +211,8 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const float2 xs = make_float2(x2[r].x + dp.x, x2[r].y + dp.y);
-                const float2 ls = make_float2(ga2[r].x - b2[r].x + cl.x, ga2[r].y - b2[r].y + cl.y);
+                const float2 gar = scr[r * 32];
+                const float2 ls = make_float2(gar.x - b2[r].x + cl.x, gar.y - b2[r].y + cl.y);
                 xl.x = fmaf(xs.x, ls.x, xl.x); xl.y = fmaf(xs.y, ls.y, xl.y);
                 sl.x += ls.x; sl.y += ls.y; sxx.x += xs.x; sxx.y += xs.y;
                 lmx.x = fmaxf(lmx.x, ls.x); lmx.y = fmaxf(lmx.y, ls.y);
@@ -244,7 +246,7 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
 #pragma unroll
                             for (int e = 0; e < 4; ++e) {
                                 const int r = t + 16 * hh + 4 * e;
-                                const float bb = H_(b2[r]), gg = H_(ga2[r]);
+                                const float bb = H_(b2[r]), gg = H_(scr[r * 32]);
                                 av[e] = flat ? (1.0f / 32.0f) : (H_(x2[r]) + xsh) * rsa;
                                 lv[e] = flat ? lam0 : (gg - bb) + lsh;
                                 // G a of the shifted, normalised point, minus b
