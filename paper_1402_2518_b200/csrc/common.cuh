@@ -31,6 +31,7 @@ struct LibView {
                         // (pos: no equality constraint, nu == 0, library not centred, G64 not shifted)
     const float *Gi;    // R x R fp32, (Gc + 1e-4 gdmax I)^-1 (start point of IPLS: regularised sum-constrained LS)
     const float *Giq;   // R, row sums of Gi
+    const float *Gpad;  // R > 64 only: Gc zero-padded to (32 ceil(R / 32))^2, identity on the padded diagonal (ipls_c256.cuh)
 };
 
 struct SolveParams {

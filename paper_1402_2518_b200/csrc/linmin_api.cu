@@ -18,6 +18,7 @@
 #include "ipls_generic.cuh"
 #include "ipls_q32.cuh"
 #include "ipls_w64.cuh"
+#include "ipls_c256.cuh"
 #include "precompute.cuh"
 #include "whiten.cuh"
 #include "detect.cuh"
@@ -42,6 +43,7 @@ struct linmin_library {
     int sm_count = 0;
     cudaStream_t stream = nullptr;   // stream the handle was created on (frees are ordered on it)
     float *A = nullptr, *At = nullptr, *Ac = nullptr, *c = nullptr, *Gc = nullptr, *Gi = nullptr, *Giq = nullptr;
+    float *Gpad = nullptr;           // more than 64 endmembers: Gc zero-padded to whole 32 x 32 blocks (ipls_c256.cuh)
     float *scal = nullptr;           // device scalars: gdmax, sum of Giq
     int *flags = nullptr;            // device word: bit 0 = non-finite library
     double *G64 = nullptr, *W64 = nullptr;
@@ -160,6 +162,7 @@ LibView view_of(const linmin_library *lib) {
     v.cons = lib->constraint != LINMIN_CONSTRAINT_POSITIVITY_ONLY;
     v.L = lib->L; v.R = lib->Ri; v.A = lib->A; v.At = lib->At; v.Ac = lib->Ac; v.c = lib->c; v.Gc = lib->Gc;
     v.G64 = lib->G64; v.scal = lib->scal; v.flags = lib->flags; v.Gi = lib->Gi; v.Giq = lib->Giq;
+    v.Gpad = lib->Gpad;
     return v;
 }
 
@@ -272,6 +275,10 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
         int grid = persistent_grid(ipls_generic_kernel<32>, block, smem, lib->sm_count, N, teams);
         ipls_generic_kernel<32><<<grid, block, smem, o.stream>>>(lv, prm);
         CK(cudaGetLastError());
+        ++launches;
+    } else if (R <= 256 && lib->Gpad && ipls_c256_fits(L, R)) {
+        // 65..256 endmembers: one CTA per pixel, blocked Cholesky with the block products on the tensor cores
+        CK(launch_ipls_c256(lv, prm, lib->sm_count, counters, o.stream));
         ++launches;
     } else {
         const int block = 256;
@@ -394,6 +401,12 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
         // start point data of IPLS: inverse of the regularised centred Gram matrix, its row sums, gdmax
         start_data_kernel<<<1, 1024, 0, stream>>>(lib->Gc, Ri, lib->W64, lib->Gi, lib->Giq, lib->scal, lib->G64, cons ? 1 : 0);
         CKF(cudaGetLastError());
+        if (Ri > 64) {
+            const int Rp = 32 * c256::nblocks(Ri);
+            CKF(cudaMallocAsync((void **)&lib->Gpad, (size_t)Rp * Rp * sizeof(float), stream));
+            pad_gram_kernel<<<(Rp * Rp + block - 1) / block, block, 0, stream>>>(lib->Gc, Ri, Rp, lib->Gpad);
+            CKF(cudaGetLastError());
+        }
     }
     cudaFreeAsync(Araw, stream); Araw = nullptr;
     if (covd) { cudaFreeAsync(covd, stream); covd = nullptr; }
@@ -462,7 +475,7 @@ void linmin_library_destroy(linmin_library *lib) {
         lib->n_use = 0;
     }
     void *bufs[] = {lib->A, lib->At, lib->Ac, lib->c, lib->Gc, lib->Gi, lib->Giq, lib->scal, lib->G64, lib->W64, lib->flags,
-                    lib->W, lib->Wd, lib->Cd};
+                    lib->W, lib->Wd, lib->Cd, lib->Gpad};
     for (void *q : bufs) if (q) cudaFreeAsync(q, s);
     for (int i = 0; i < 3; ++i) if (lib->ev[i]) cudaEventDestroy(lib->ev[i]);
     (void)cudaGetLastError();
