@@ -29,16 +29,17 @@ constexpr unsigned FULL = 0xffffffffu;
 
 __host__ __device__ inline int nblocks(int R) { return (R + 31) >> 5; }
 __host__ __device__ inline int blk(int I, int J) { return (I * (I + 1) / 2 + J) * BLK; }      // I >= J
-// shared memory (floats): blocks | yc[L4] | xs0[Rp] | xs1[Rp] | dgs[Rp] | line[64] | red[64]
+// shared memory (floats): blocks | yc[L4] | xs0[Rp] | xs1[Rp] | dgs[Rp] | line[128] | red[64]
 __host__ __device__ inline size_t smem_floats(int L, int R) {
     const int NB = nblocks(R), Rp = 32 * NB, L4 = (L + 3) & ~3;
-    return (size_t)(NB * (NB + 1) / 2) * BLK + L4 + 3 * (size_t)Rp + 128;
+    return (size_t)(NB * (NB + 1) / 2) * BLK + L4 + 3 * (size_t)Rp + 192;
 }
 
+// x = big + small with big the leading 11 significand bits (the tensor core reads the upper 19 bits of a tf32 operand, so
+// `small` needs no rounding of its own: 22 of the 24 bits take part; cvt.rna.tf32 is a 6-instruction emulation here)
 __device__ __forceinline__ void split_tf32(float x, uint32_t &big, uint32_t &small) {
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(big) : "f"(x));
-    const float r = x - __uint_as_float(big);
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(small) : "f"(r));
+    big = __float_as_uint(x) & 0xffffe000u;
+    small = __float_as_uint(x - __uint_as_float(big));
 }
 __device__ __forceinline__ void mma_tf32(float (&c)[4], const uint32_t (&a)[4], const uint32_t (&b)[2]) {
     asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
@@ -46,19 +47,20 @@ __device__ __forceinline__ void mma_tf32(float (&c)[4], const uint32_t (&a)[4], 
                  : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
 }
 
-// C (32 x 32) = [C +] sign X Y' for one warp; X, Y, C blocks of stride BS (C may alias X: X is read in full first)
-template <bool ACCUM>
-__device__ __forceinline__ void block_product(float *C, const float *X, const float *Y, float sign, int lane) {
+// One warp: C = X Y' (UPDATE false) or C -= X Y' (UPDATE true: accumulates X Y' - C and stores the negative);
+// X, Y, C are 32 x 32 blocks of stride BS; C may alias X (X is read in full first)
+template <bool UPDATE>
+__device__ __forceinline__ void block_product(float *C, const float *X, const float *Y, int lane) {
     const int g = lane >> 2, t = lane & 3;
     float acc[2][4][4];
 #pragma unroll
     for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
         for (int nt = 0; nt < 4; ++nt) {
-            if (ACCUM) {
+            if (UPDATE) {
                 const float2 lo = *reinterpret_cast<const float2 *>(C + (16 * mt + g) * BS + 8 * nt + 2 * t);
                 const float2 hi = *reinterpret_cast<const float2 *>(C + (16 * mt + g + 8) * BS + 8 * nt + 2 * t);
-                acc[mt][nt][0] = lo.x; acc[mt][nt][1] = lo.y; acc[mt][nt][2] = hi.x; acc[mt][nt][3] = hi.y;
+                acc[mt][nt][0] = -lo.x; acc[mt][nt][1] = -lo.y; acc[mt][nt][2] = -hi.x; acc[mt][nt][3] = -hi.y;
             } else {
                 acc[mt][nt][0] = acc[mt][nt][1] = acc[mt][nt][2] = acc[mt][nt][3] = 0.0f;
             }
@@ -69,10 +71,10 @@ __device__ __forceinline__ void block_product(float *C, const float *X, const fl
 #pragma unroll
         for (int mt = 0; mt < 2; ++mt) {
             const float *x = X + (16 * mt + g) * BS + 8 * ks + t;
-            split_tf32(sign * x[0], ab[ks][mt][0], as[ks][mt][0]);
-            split_tf32(sign * x[8 * BS], ab[ks][mt][1], as[ks][mt][1]);
-            split_tf32(sign * x[4], ab[ks][mt][2], as[ks][mt][2]);
-            split_tf32(sign * x[8 * BS + 4], ab[ks][mt][3], as[ks][mt][3]);
+            split_tf32(x[0], ab[ks][mt][0], as[ks][mt][0]);
+            split_tf32(x[8 * BS], ab[ks][mt][1], as[ks][mt][1]);
+            split_tf32(x[4], ab[ks][mt][2], as[ks][mt][2]);
+            split_tf32(x[8 * BS + 4], ab[ks][mt][3], as[ks][mt][3]);
         }
 #pragma unroll
     for (int ks = 0; ks < 4; ++ks) {
@@ -95,86 +97,155 @@ __device__ __forceinline__ void block_product(float *C, const float *X, const fl
     for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
         for (int nt = 0; nt < 4; ++nt) {
-            *reinterpret_cast<float2 *>(C + (16 * mt + g) * BS + 8 * nt + 2 * t) = make_float2(acc[mt][nt][0], acc[mt][nt][1]);
-            *reinterpret_cast<float2 *>(C + (16 * mt + g + 8) * BS + 8 * nt + 2 * t) = make_float2(acc[mt][nt][2], acc[mt][nt][3]);
+            const float sg = UPDATE ? -1.0f : 1.0f;
+            *reinterpret_cast<float2 *>(C + (16 * mt + g) * BS + 8 * nt + 2 * t) = make_float2(sg * acc[mt][nt][0], sg * acc[mt][nt][1]);
+            *reinterpret_cast<float2 *>(C + (16 * mt + g + 8) * BS + 8 * nt + 2 * t) = make_float2(sg * acc[mt][nt][2], sg * acc[mt][nt][3]);
         }
 }
 
-// One warp: Cholesky factor of the 32 x 32 diagonal block B (lower triangle read), then B <- W = L^-1 (lower, zeros
-// above the diagonal).  Lane i holds row i; step j sends column j through `line` (two halves, alternating).
-// A pivot below floorv is clamped (returns true if that happened).
-__device__ __forceinline__ bool factor_diag(float *B, float *line, float floorv, int lane) {
-    float m[32];
+// One warp: B <- W = L^-1 (lower triangular, zeros above the diagonal) for the Cholesky factor L of the 32 x 32 diagonal
+// block B (read in full: it is symmetric).  B = L~ D L~' with L~ = E_0 E_1 .. E_30, E_j = I + l_j e_j' (l_j: the
+// multipliers of step j), so L~^-T = (I - e_0 l_0')(I - e_1 l_1') .. : lane i holds row i of the Schur complement (m) and
+// row i of U = L~^-T (u), and step j is, for both, "entry k -= (entry j / p_j) c_k" with c = column j of the Schur
+// complement -- which every lane contributes ONE element of (one conflict-free store, then eight broadcast loads).
+// Both rows are kept shifted so that entry j sits in register 0 (each FMA writes one register to the left: no register
+// index depends on j, no moves), the column is stored rotated the same way, and the loop is ROLLED on purpose: fully
+// unrolled, the sweep was 32 KB of straight-line code run by a single warp and took 11.8 k cycles per block, one
+// instruction-cache miss per 128-byte line.  Column j of U is final at step j and goes straight to row j of W,
+// scaled by p_j^-1/2 (W = D^-1/2 L~^-1).  A pivot below floorv is clamped (returns true if that happened).
+// The sweep is shared by TWO warps (role 0: the rows m and the column exchange; role 1: the rows u and the output), which
+// meet at named barrier 1 once per step: 31 FMAs per step and warp instead of 62 on the dependent chain.
+__device__ __forceinline__ bool factor_diag(float *B, float *line, float floorv, int lane, int role) {
+    float v[32];                                          // role 0: row `lane` of m; role 1: row `lane` of u
+    if (role == 0) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const float4 x = *reinterpret_cast<const float4 *>(B + lane * BS + 4 * q);
+            v[4 * q] = x.x; v[4 * q + 1] = x.y; v[4 * q + 2] = x.z; v[4 * q + 3] = x.w;
+        }
+        line[lane] = v[0];
+    } else {
+#pragma unroll
+        for (int k = 0; k < 32; ++k) v[k] = (k == lane) ? 1.0f : 0.0f;
+    }
+    bool clamped = false;
+    float c[32];
+    asm volatile("bar.sync 1, 64;" ::: "memory");         // (also: B has been read in full; row j is written at step j)
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
-        const float4 v = *reinterpret_cast<const float4 *>(B + lane * BS + 4 * q);
-        m[4 * q] = v.x; m[4 * q + 1] = v.y; m[4 * q + 2] = v.z; m[4 * q + 3] = v.w;
+        const float4 c4 = *reinterpret_cast<const float4 *>(line + 4 * q);
+        c[4 * q] = c4.x; c[4 * q + 1] = c4.y; c[4 * q + 2] = c4.z; c[4 * q + 3] = c4.w;
     }
-    bool clamped = false;
-#pragma unroll
+    // software pipeline: the entry of column j + 1 is computed, stored and the next line requested BEFORE the FMAs of
+    // step j, which then cover the store-to-load round trip.  (Taking the next pivot from its owner by shuffle, to get the
+    // reciprocal off the chain, was slower: 5.2 k -> 8 k cycles per block.)
+#pragma unroll 2
     for (int j = 0; j < 32; ++j) {
-        float *cb = line + 32 * (j & 1);
-        cb[lane] = m[j];                         // column j of the Schur complement (rows >= j matter)
-        __syncwarp();
-        float pj = cb[j];
+        float pj = c[0];
         if (!(pj > floorv)) { pj = floorv; clamped = true; }
-        const float li = m[j] * rcp_approx(pj);
+        const float lv = -v[0] * rcp_approx(pj);
+        float *cbn = line + 32 * ((j + 1) & 1);
+        if (role == 0) cbn[(lane - j - 1) & 31] = fmaf(lv, c[1], v[1]);   // column j + 1, rotated: index r = row j + 1 + r
+        else B[j * BS + lane] = v[0] * rsqrtf(pj);
+        asm volatile("bar.sync 1, 64;" ::: "memory");
+        float cn[32];
 #pragma unroll
-        for (int q = (j + 1) / 4; q < 8; ++q) {
-            const float4 c4 = *reinterpret_cast<const float4 *>(cb + 4 * q);
-            if (4 * q + 0 > j) m[4 * q + 0] = fmaf(-li, c4.x, m[4 * q + 0]);
-            if (4 * q + 1 > j) m[4 * q + 1] = fmaf(-li, c4.y, m[4 * q + 1]);
-            if (4 * q + 2 > j) m[4 * q + 2] = fmaf(-li, c4.z, m[4 * q + 2]);
-            if (4 * q + 3 > j) m[4 * q + 3] = fmaf(-li, c4.w, m[4 * q + 3]);
+        for (int q = 0; q < 8; ++q) {
+            const float4 c4 = *reinterpret_cast<const float4 *>(cbn + 4 * q);
+            cn[4 * q] = c4.x; cn[4 * q + 1] = c4.y; cn[4 * q + 2] = c4.z; cn[4 * q + 3] = c4.w;
         }
-        const float rs = rsqrtf(pj);
-        m[j] = (lane == j) ? pj * rs : m[j] * rs;     // L_ij (rows > j), L_jj = sqrt(p_j)
+#pragma unroll
+        for (int r = 1; r < 32; ++r) v[r - 1] = fmaf(lv, c[r], v[r]);
+        v[31] = 0.0f;
+#pragma unroll
+        for (int r = 0; r < 32; ++r) c[r] = cn[r];
     }
-    __syncwarp();
-#pragma unroll
-    for (int q = 0; q < 8; ++q)
-        *reinterpret_cast<float4 *>(B + lane * BS + 4 * q) = make_float4(m[4 * q], m[4 * q + 1], m[4 * q + 2], m[4 * q + 3]);
-    __syncwarp();
-    // W = L^-1: lane c solves L w = e_c by forward substitution (rows of L broadcast from shared memory)
-    float w[32];
-#pragma unroll
-    for (int i = 0; i < 32; ++i) {
-        float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f, s3 = 0.0f, lii = 1.0f;
-#pragma unroll
-        for (int q = 0; q <= i / 4; ++q) {
-            const float4 l4 = *reinterpret_cast<const float4 *>(B + i * BS + 4 * q);
-            if (4 * q + 0 < i) s0 = fmaf(l4.x, w[4 * q + 0], s0); else if (4 * q + 0 == i) lii = l4.x;
-            if (4 * q + 1 < i) s1 = fmaf(l4.y, w[4 * q + 1], s1); else if (4 * q + 1 == i) lii = l4.y;
-            if (4 * q + 2 < i) s2 = fmaf(l4.z, w[4 * q + 2], s2); else if (4 * q + 2 == i) lii = l4.z;
-            if (4 * q + 3 < i) s3 = fmaf(l4.w, w[4 * q + 3], s3); else if (4 * q + 3 == i) lii = l4.w;
-        }
-        const float e = (lane == i) ? 1.0f : 0.0f;
-        w[i] = (e - ((s0 + s1) + (s2 + s3))) * rcp_approx(lii);
-    }
-    __syncwarp();                                // every lane has read L
-#pragma unroll
-    for (int i = 0; i < 32; ++i) B[i * BS + lane] = w[i];
     return clamped;
 }
 
+#ifdef C256_PROFILE
+__device__ long long c256_prof_g[8];
+#define c256_prof c256_prof_l
+#endif
 // In-place blocked Cholesky of the block lower triangle; on return block (p, p) holds W_pp = L_pp^-1 and the blocks
 // below the diagonal hold L.  All 256 threads call it.
-__device__ __forceinline__ bool factor_blocks(float *Mb, float *line, int NB, float floorv, int warp, int lane) {
+__device__ __forceinline__ bool factor_blocks(float *Mb, float *line, int NB, float floorv, int warp, int lane
+#ifdef C256_PROFILE
+    , long long *c256_prof_l
+#endif
+) {
     bool clamped = false;
+    // Look-ahead: once the blocks of column p + 1 have their update of panel p, warps 0 and 1 factor the next diagonal
+    // block while the other warps finish the trailing update (the diagonal sweep is 32 dependent steps of one warp).
+    if (warp < 2) clamped |= factor_diag(Mb + blk(0, 0), line, floorv, lane, warp);
+    __syncthreads();
     for (int p = 0; p < NB; ++p) {
-        if (warp == 0) clamped |= factor_diag(Mb + blk(p, p), line, floorv, lane);
-        __syncthreads();
+#ifdef C256_PROFILE
+        long long t0 = clock64();
+#endif
         for (int I = p + 1 + warp; I < NB; I += NT / 32)
-            block_product<false>(Mb + blk(I, p), Mb + blk(I, p), Mb + blk(p, p), 1.0f, lane);
+            block_product<false>(Mb + blk(I, p), Mb + blk(I, p), Mb + blk(p, p), lane);
         __syncthreads();
-        int n = 0;
-        for (int J = p + 1; J < NB; ++J)
-            for (int I = J; I < NB; ++I, ++n)
-                if ((n & (NT / 32 - 1)) == warp)
-                    block_product<true>(Mb + blk(I, J), Mb + blk(I, p), Mb + blk(J, p), -1.0f, lane);
+#ifdef C256_PROFILE
+        long long t1 = clock64(); c256_prof[1] += t1 - t0;
+#endif
+        if (p + 1 >= NB) break;
+        for (int I = p + 1 + warp; I < NB; I += NT / 32)               // column p + 1 first
+            block_product<true>(Mb + blk(I, p + 1), Mb + blk(I, p), Mb + blk(p + 1, p), lane);
         __syncthreads();
+#ifdef C256_PROFILE
+        t0 = clock64(); c256_prof[0] += t0 - t1;
+#endif
+        if (warp < 2) {
+            clamped |= factor_diag(Mb + blk(p + 1, p + 1), line, floorv, lane, warp);
+        } else {
+            int n = 0;
+            for (int J = p + 2; J < NB; ++J)
+                for (int I = J; I < NB; ++I, ++n)
+                    if (n % (NT / 32 - 2) == warp - 2)
+                        block_product<true>(Mb + blk(I, J), Mb + blk(I, p), Mb + blk(J, p), lane);
+        }
+        __syncthreads();
+#ifdef C256_PROFILE
+        t1 = clock64(); c256_prof[2] += t1 - t0;
+#endif
     }
     return clamped;
+}
+
+// dot products of one 32-float row (16-byte loads) with one or two 32-float vectors, four accumulators each
+template <int NRHS>
+__device__ __forceinline__ void row_dot(const float *row, const float *v0, const float *v1, float &r0, float &r1) {
+    float s[4] = {0.0f, 0.0f, 0.0f, 0.0f}, u[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const float4 a4 = *reinterpret_cast<const float4 *>(row + 4 * q);
+        const float4 x4 = *reinterpret_cast<const float4 *>(v0 + 4 * q);
+        s[0] = fmaf(a4.x, x4.x, s[0]); s[1] = fmaf(a4.y, x4.y, s[1]); s[2] = fmaf(a4.z, x4.z, s[2]); s[3] = fmaf(a4.w, x4.w, s[3]);
+        if (NRHS > 1) {
+            const float4 y4 = *reinterpret_cast<const float4 *>(v1 + 4 * q);
+            u[0] = fmaf(a4.x, y4.x, u[0]); u[1] = fmaf(a4.y, y4.y, u[1]); u[2] = fmaf(a4.z, y4.z, u[2]); u[3] = fmaf(a4.w, y4.w, u[3]);
+        }
+    }
+    r0 = (s[0] + s[1]) + (s[2] + s[3]);
+    r1 = (u[0] + u[1]) + (u[2] + u[3]);
+}
+// the same down one column of a block (element k at col[k BS])
+template <int NRHS>
+__device__ __forceinline__ void col_dot(const float *col, const float *v0, const float *v1, float &r0, float &r1) {
+    float s[4] = {0.0f, 0.0f, 0.0f, 0.0f}, u[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const float4 x4 = *reinterpret_cast<const float4 *>(v0 + 4 * q);
+        const float a0 = col[(4 * q + 0) * BS], a1 = col[(4 * q + 1) * BS], a2 = col[(4 * q + 2) * BS], a3 = col[(4 * q + 3) * BS];
+        s[0] = fmaf(a0, x4.x, s[0]); s[1] = fmaf(a1, x4.y, s[1]); s[2] = fmaf(a2, x4.z, s[2]); s[3] = fmaf(a3, x4.w, s[3]);
+        if (NRHS > 1) {
+            const float4 y4 = *reinterpret_cast<const float4 *>(v1 + 4 * q);
+            u[0] = fmaf(a0, y4.x, u[0]); u[1] = fmaf(a1, y4.y, u[1]); u[2] = fmaf(a2, y4.z, u[2]); u[3] = fmaf(a3, y4.w, u[3]);
+        }
+    }
+    r0 = (s[0] + s[1]) + (s[2] + s[3]);
+    r1 = (u[0] + u[1]) + (u[2] + u[3]);
 }
 
 // (L L') x = rhs in place for NRHS right-hand sides (x0, x1: Rp floats each in shared memory); thread t owns row t.
@@ -185,36 +256,16 @@ __device__ __forceinline__ void solve_blocks(const float *Mb, int NB, float *x0,
     // ---- forward, L z = r:  z_p = W_pp r_p, then r_q -= L_qp z_p for q > p
     for (int p = 0; p < NB; ++p) {
         if (I == p) {
-            const float *wr = Mb + blk(p, p) + i * BS;
-            float s0 = 0.0f, s1 = 0.0f;
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                const float4 w4 = *reinterpret_cast<const float4 *>(wr + 4 * q);
-                const float4 r4 = *reinterpret_cast<const float4 *>(x0 + 32 * p + 4 * q);
-                s0 = fmaf(w4.x, r4.x, s0); s0 = fmaf(w4.y, r4.y, s0); s0 = fmaf(w4.z, r4.z, s0); s0 = fmaf(w4.w, r4.w, s0);
-                if (NRHS > 1) {
-                    const float4 q4 = *reinterpret_cast<const float4 *>(x1 + 32 * p + 4 * q);
-                    s1 = fmaf(w4.x, q4.x, s1); s1 = fmaf(w4.y, q4.y, s1); s1 = fmaf(w4.z, q4.z, s1); s1 = fmaf(w4.w, q4.w, s1);
-                }
-            }
+            float s0, s1;
+            row_dot<NRHS>(Mb + blk(p, p) + i * BS, x0 + 32 * p, x1 + 32 * p, s0, s1);
             __syncwarp();
             x0[tid] = s0;
             if (NRHS > 1) x1[tid] = s1;
         }
         __syncthreads();
         if (I > p && I < NB) {
-            const float *lr = Mb + blk(I, p) + i * BS;
-            float s0 = 0.0f, s1 = 0.0f;
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                const float4 l4 = *reinterpret_cast<const float4 *>(lr + 4 * q);
-                const float4 z4 = *reinterpret_cast<const float4 *>(x0 + 32 * p + 4 * q);
-                s0 = fmaf(l4.x, z4.x, s0); s0 = fmaf(l4.y, z4.y, s0); s0 = fmaf(l4.z, z4.z, s0); s0 = fmaf(l4.w, z4.w, s0);
-                if (NRHS > 1) {
-                    const float4 y4 = *reinterpret_cast<const float4 *>(x1 + 32 * p + 4 * q);
-                    s1 = fmaf(l4.x, y4.x, s1); s1 = fmaf(l4.y, y4.y, s1); s1 = fmaf(l4.z, y4.z, s1); s1 = fmaf(l4.w, y4.w, s1);
-                }
-            }
+            float s0, s1;
+            row_dot<NRHS>(Mb + blk(I, p) + i * BS, x0 + 32 * p, x1 + 32 * p, s0, s1);
             x0[tid] -= s0;
             if (NRHS > 1) x1[tid] -= s1;
         }
@@ -225,28 +276,16 @@ __device__ __forceinline__ void solve_blocks(const float *Mb, int NB, float *x0,
     // ---- backward, L' x = z:  x_p = W_pp' z_p, then z_q -= L_pq' x_p for q < p
     for (int p = NB - 1; p >= 0; --p) {
         if (I == p) {
-            const float *wc = Mb + blk(p, p) + i;
-            float s0 = 0.0f, s1 = 0.0f;
-#pragma unroll 8
-            for (int k = 0; k < 32; ++k) {
-                const float wv = wc[k * BS];
-                s0 = fmaf(wv, x0[32 * p + k], s0);
-                if (NRHS > 1) s1 = fmaf(wv, x1[32 * p + k], s1);
-            }
+            float s0, s1;
+            col_dot<NRHS>(Mb + blk(p, p) + i, x0 + 32 * p, x1 + 32 * p, s0, s1);
             __syncwarp();
             x0[tid] = s0;
             if (NRHS > 1) x1[tid] = s1;
         }
         __syncthreads();
         if (I < p) {
-            const float *lc = Mb + blk(p, I) + i;
-            float s0 = 0.0f, s1 = 0.0f;
-#pragma unroll 8
-            for (int k = 0; k < 32; ++k) {
-                const float lv = lc[k * BS];
-                s0 = fmaf(lv, x0[32 * p + k], s0);
-                if (NRHS > 1) s1 = fmaf(lv, x1[32 * p + k], s1);
-            }
+            float s0, s1;
+            col_dot<NRHS>(Mb + blk(p, I) + i, x0 + 32 * p, x1 + 32 * p, s0, s1);
             x0[tid] -= s0;
             if (NRHS > 1) x1[tid] -= s1;
         }
@@ -324,7 +363,7 @@ ipls_c256_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counte
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     float *Mb = smem;
     float *yc = Mb + (size_t)(NB * (NB + 1) / 2) * BLK;
-    float *xs0 = yc + L4, *xs1 = xs0 + Rp, *dgs = xs1 + Rp, *line = dgs + Rp, *redm = line + 64;
+    float *xs0 = yc + L4, *xs1 = xs0 + Rp, *dgs = xs1 + Rp, *line = dgs + Rp, *redm = line + 128;
     const Red rd{redm, warp, lane};
     __shared__ unsigned int s_ticket;
     const float gdmax = lib.scal[0];
@@ -333,6 +372,10 @@ ipls_c256_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counte
     const bool cons = lib.cons != 0;
     const float giq = live ? lib.Giq[tid] : 0.0f;
 
+#ifdef C256_PROFILE
+    long long prof[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long tK0 = clock64();
+#endif
     while (true) {
         if (tid == 0) s_ticket = atomicAdd(counter, 1u);
         __syncthreads();
@@ -436,7 +479,9 @@ ipls_c256_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counte
             if (!live) { a = 1.0f; lam = 0.0f; Ga = 0.0f; }
         }
         int iters = 0, flags = 0;
-
+#ifdef C256_PROFILE
+        long long tI0 = clock64();
+#endif
         for (int it = 0;; ++it) {
             // ---- residuals
             const float w = Ga - b + nu;          // G a is carried along with a (Newton identity, see the update)
@@ -470,7 +515,13 @@ ipls_c256_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counte
                 if (tid < Rp) Mb[blk(warp, warp) + lane * BS + lane] += di;
                 __syncthreads();
             }
+#ifdef C256_PROFILE
+            long long tA = clock64();
+            if (factor_blocks(Mb, line, NB, 1e-12f * gdmax, warp, lane, prof)) flags |= LINMIN_INFO_CHOL_REGULARISED;
+            long long tB = clock64(); prof[3] += tB - tA;
+#else
             if (factor_blocks(Mb, line, NB, 1e-12f * gdmax, warp, lane)) flags |= LINMIN_INFO_CHOL_REGULARISED;
+#endif
             // ---- predictor
             if (tid < Rp) { xs0[tid] = live ? -w : 0.0f; xs1[tid] = live ? 1.0f : 0.0f; }
             __syncthreads();
@@ -511,10 +562,18 @@ ipls_c256_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counte
             }
             nu = fmaf(ad, dnu, nu);
         }
+#ifdef C256_PROFILE
+        prof[4] += clock64() - tI0; prof[5] += iters;
+#endif
         // hand-over: zero where the primal-dual indicator says inactive (LINMIN_TAPIA_KAPPA, common.cuh)
         if (live) prm.coeffs[p * R + tid] = (a * sc > LINMIN_TAPIA_KAPPA * lam) ? a : 0.0f;
         if (prm.info && tid == 0) prm.info[p] = flags | (iters << 8);
     }
+#ifdef C256_PROFILE
+    if (blockIdx.x == 0 && tid == 0)
+        printf("c256 cycles: total %lld iterloop %lld factor %lld (diag %lld trsm %lld update %lld) iters %lld\n",
+               clock64() - tK0, prof[4], prof[3], prof[0], prof[1], prof[2], prof[5]);
+#endif
 }
 
 inline cudaError_t launch_ipls_c256(const LibView &lv, const SolveParams &prm, int sm_count, unsigned int *counter,

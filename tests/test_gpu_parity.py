@@ -282,7 +282,8 @@ def test_scale_and_offset_invariance(lm):
     np.testing.assert_allclose(go["coeffs"], g["coeffs"], atol=2e-5)
 
 
-@pytest.mark.parametrize("L,R", [(110, 36), (56, 36), (33, 5), (200, 100), (110, 32), (240, 20), (400, 12), (512, 32)])
+@pytest.mark.parametrize("L,R", [(110, 36), (56, 36), (33, 5), (200, 100), (110, 32), (240, 20), (400, 12), (512, 32),
+                                 (150, 65), (260, 129), (240, 255)])
 def test_odd_sizes(lm, L, R):
     """The paper's own sizes (110 or 56 channels, 36 endmembers) and others."""
     import oracle
