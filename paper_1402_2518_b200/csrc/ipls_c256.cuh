@@ -163,39 +163,22 @@ __device__ __forceinline__ bool factor_diag(float *B, float *line, float floorv,
     return clamped;
 }
 
-#ifdef C256_PROFILE
-__device__ long long c256_prof_g[8];
-#define c256_prof c256_prof_l
-#endif
 // In-place blocked Cholesky of the block lower triangle; on return block (p, p) holds W_pp = L_pp^-1 and the blocks
 // below the diagonal hold L.  All 256 threads call it.
-__device__ __forceinline__ bool factor_blocks(float *Mb, float *line, int NB, float floorv, int warp, int lane
-#ifdef C256_PROFILE
-    , long long *c256_prof_l
-#endif
-) {
+__device__ __forceinline__ bool factor_blocks(float *Mb, float *line, int NB, float floorv, int warp, int lane) {
     bool clamped = false;
     // Look-ahead: once the blocks of column p + 1 have their update of panel p, warps 0 and 1 factor the next diagonal
-    // block while the other warps finish the trailing update (the diagonal sweep is 32 dependent steps of one warp).
+    // block while the other warps finish the trailing update (the diagonal sweep is 32 dependent steps).
     if (warp < 2) clamped |= factor_diag(Mb + blk(0, 0), line, floorv, lane, warp);
     __syncthreads();
     for (int p = 0; p < NB; ++p) {
-#ifdef C256_PROFILE
-        long long t0 = clock64();
-#endif
         for (int I = p + 1 + warp; I < NB; I += NT / 32)
             block_product<false>(Mb + blk(I, p), Mb + blk(I, p), Mb + blk(p, p), lane);
         __syncthreads();
-#ifdef C256_PROFILE
-        long long t1 = clock64(); c256_prof[1] += t1 - t0;
-#endif
         if (p + 1 >= NB) break;
         for (int I = p + 1 + warp; I < NB; I += NT / 32)               // column p + 1 first
             block_product<true>(Mb + blk(I, p + 1), Mb + blk(I, p), Mb + blk(p + 1, p), lane);
         __syncthreads();
-#ifdef C256_PROFILE
-        t0 = clock64(); c256_prof[0] += t0 - t1;
-#endif
         if (warp < 2) {
             clamped |= factor_diag(Mb + blk(p + 1, p + 1), line, floorv, lane, warp);
         } else {
@@ -206,9 +189,6 @@ __device__ __forceinline__ bool factor_blocks(float *Mb, float *line, int NB, fl
                         block_product<true>(Mb + blk(I, J), Mb + blk(I, p), Mb + blk(J, p), lane);
         }
         __syncthreads();
-#ifdef C256_PROFILE
-        t1 = clock64(); c256_prof[2] += t1 - t0;
-#endif
     }
     return clamped;
 }
@@ -372,10 +352,6 @@ ipls_c256_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counte
     const bool cons = lib.cons != 0;
     const float giq = live ? lib.Giq[tid] : 0.0f;
 
-#ifdef C256_PROFILE
-    long long prof[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    long long tK0 = clock64();
-#endif
     while (true) {
         if (tid == 0) s_ticket = atomicAdd(counter, 1u);
         __syncthreads();
@@ -479,9 +455,6 @@ ipls_c256_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counte
             if (!live) { a = 1.0f; lam = 0.0f; Ga = 0.0f; }
         }
         int iters = 0, flags = 0;
-#ifdef C256_PROFILE
-        long long tI0 = clock64();
-#endif
         for (int it = 0;; ++it) {
             // ---- residuals
             const float w = Ga - b + nu;          // G a is carried along with a (Newton identity, see the update)
@@ -515,13 +488,7 @@ ipls_c256_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counte
                 if (tid < Rp) Mb[blk(warp, warp) + lane * BS + lane] += di;
                 __syncthreads();
             }
-#ifdef C256_PROFILE
-            long long tA = clock64();
-            if (factor_blocks(Mb, line, NB, 1e-12f * gdmax, warp, lane, prof)) flags |= LINMIN_INFO_CHOL_REGULARISED;
-            long long tB = clock64(); prof[3] += tB - tA;
-#else
             if (factor_blocks(Mb, line, NB, 1e-12f * gdmax, warp, lane)) flags |= LINMIN_INFO_CHOL_REGULARISED;
-#endif
             // ---- predictor
             if (tid < Rp) { xs0[tid] = live ? -w : 0.0f; xs1[tid] = live ? 1.0f : 0.0f; }
             __syncthreads();
@@ -562,18 +529,10 @@ ipls_c256_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counte
             }
             nu = fmaf(ad, dnu, nu);
         }
-#ifdef C256_PROFILE
-        prof[4] += clock64() - tI0; prof[5] += iters;
-#endif
         // hand-over: zero where the primal-dual indicator says inactive (LINMIN_TAPIA_KAPPA, common.cuh)
         if (live) prm.coeffs[p * R + tid] = (a * sc > LINMIN_TAPIA_KAPPA * lam) ? a : 0.0f;
         if (prm.info && tid == 0) prm.info[p] = flags | (iters << 8);
     }
-#ifdef C256_PROFILE
-    if (blockIdx.x == 0 && tid == 0)
-        printf("c256 cycles: total %lld iterloop %lld factor %lld (diag %lld trsm %lld update %lld) iters %lld\n",
-               clock64() - tK0, prof[4], prof[3], prof[0], prof[1], prof[2], prof[5]);
-#endif
 }
 
 inline cudaError_t launch_ipls_c256(const LibView &lv, const SolveParams &prm, int sm_count, unsigned int *counter,
