@@ -80,8 +80,13 @@ extern "C" {
  * linmin_library_create reads it from opts, linmin_unmix_lib requires the same value (or opts == NULL). */
 #define LINMIN_CONSTRAINT_SUM_TO_ONE 0        /* eq. 3 + eq. 4: the hot path */
 #define LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE 1 /* a >= 0, sum a <= 1: sum-to-one with a slack (all-zero) endmember,
-                                                  added BEFORE the centring; the slack is not returned */
-#define LINMIN_CONSTRAINT_POSITIVITY_ONLY 2    /* eq. 3 only (NNLS): no centring, no equality constraint */
+                                                  added BEFORE the centring; the slack is not returned.  At R = 32
+                                                  (L <= 256) the same minimiser is computed without a slack: the
+                                                  positivity-only result where its sum is <= 1, else the sum-to-one
+                                                  result (the problem is convex: the bound is active there) */
+#define LINMIN_CONSTRAINT_POSITIVITY_ONLY 2    /* eq. 3 only (NNLS): no centring, no equality constraint.  gap_tol
+                                                  and feas_tol are applied at 1/100 of their value (the projections
+                                                  of an uncentred library overstate the scale of the gradients) */
 
 /* weighting (sec. 2.3, eq. 5-6: the renormalised problem).  Also a property of the handle.
  * With a covariance, eq. 2 is solved on the whitened data X' = X.L, S' = S.L (C^-1 = L.L^T); the `sigma`

@@ -36,7 +36,9 @@ __host__ __device__ inline size_t finish_warp_bytes(int L, int R, int KMAX) {
 }
 
 // state[i]: 0 free, 1 in F, 2 blocked (rejected as rank-deficient or degenerate tie)
-__global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams prm, int KMAX) {
+// list: NULL = all pixels; else [0] = count, [1 + i] = pixel (the overflow list of finish_sweep_kernel)
+__global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams prm, int KMAX,
+                                                     const unsigned int *__restrict__ list) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (lib.flags[0]) return;
     const int L = lib.L, R = lib.R;
@@ -55,7 +57,9 @@ __global__ void __launch_bounds__(256) finish_kernel(LibView lib, SolveParams pr
     const int max_pivots = 4 * KMAX + 8;
     const bool cons = lib.cons != 0;      // false: positivity only (no equality constraint; the empty support is feasible)
 
-    for (int64_t p = (int64_t)blockIdx.x * warps + warp; p < prm.N; p += (int64_t)gridDim.x * warps) {
+    const int64_t count = list ? (int64_t)list[0] : prm.N;
+    for (int64_t pi = (int64_t)blockIdx.x * warps + warp; pi < count; pi += (int64_t)gridDim.x * warps) {
+        const int64_t p = list ? (int64_t)list[1 + pi] : pi;
         float *cout = prm.coeffs + p * R;
         int info = prm.info ? prm.info[p] : 0;
         // ---- load y; detect non-finite

@@ -132,6 +132,9 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
     const bool csvec_ok = ((R & 3) == 0) && ((reinterpret_cast<uintptr_t>(prm.coeff_sigma) & 15) == 0);
     const float qnan = __int_as_float(0x7fc00000);
     const int max_pivots = 4 * RP + 8;
+    // false: positivity only: no equality constraint -- no normalisation, mu == nu == 0, H = K, and the
+    // empty support is feasible (a = 0)
+    const bool cons = lib.cons != 0;
     double *M0 = Md + t * MS;          // my rows of the swept matrix
     double *M1 = Md + (t + 8) * MS;
 
@@ -245,7 +248,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             for (int q = 0; q < 4; ++q) nib |= (ai[q] > LINMIN_SUPPORT_THRESHOLD && 4 * t + q < R) ? (1u << q) : 0u;
             unsigned mask = gor(nib << (4 * t));
             float best = gmaxf(fmaxf(fmaxf(ai[0], ai[1]), fmaxf(ai[2], ai[3])));
-            if (mask == 0u) {   // can not happen for a point of the simplex; be safe: the largest entry
+            if (mask == 0u && cons) {   // can not happen for a point of the simplex; be safe: the largest entry
                 unsigned nb = 0;
 #pragma unroll
                 for (int q = 0; q < 4; ++q) nb |= (ai[q] == best && 4 * t + q < R) ? (1u << q) : 0u;
@@ -296,7 +299,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
         }
         {
             const double s = gsum(a0 + a1);
-            if (st == 0) {
+            if (st == 0 && cons) {
                 const double rs = rcp_d(s);
                 a0 *= rs; a1 *= rs;
                 if (t < k) aFs[t] = a0;
@@ -438,16 +441,18 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 }
                 const double s = gsum(a0 + a1);
                 if (act && rej >= 0) {
-                    if (k == 0) {
+                    if (k == 0 && cons) {
                         // the only member was rejected (a zero endmember): stay on the simplex with it, uncertified
                         k = 1; i0 = (t == 0) ? irej : 0; a0 = (t == 0) ? 1.0 : 0.0;
                         if (t == 0) { idx[0] = irej; aFs[0] = 1.0; state[irej] = 1; }
                         st = 2; fell = true;
                     } else {
-                        const double rs = rcp_d(s);
-                        a0 *= rs; a1 *= rs;
-                        if (t < k) aFs[t] = a0;
-                        if (t + 8 < k) aFs[t + 8] = a1;
+                        if (cons) {
+                            const double rs = rcp_d(s);
+                            a0 *= rs; a1 *= rs;
+                            if (t < k) aFs[t] = a0;
+                            if (t + 8 < k) aFs[t + 8] = a1;
+                        }
                         if (pivots > max_pivots) { st = 2; fell = true; }
                     }
                 }
@@ -479,7 +484,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
             const double sx = gsum(x0 + x1);
             bool accepted = false;
             {
-                const double mu = (sx - 1.0) * rcp_d(skip ? 1.0 : sqn);
+                const double mu = cons ? (sx - 1.0) * rcp_d(skip ? 1.0 : sqn) : 0.0;
                 const double t0v = x0 - mu * q0, t1v = x1 - mu * q1;
                 const bool m0 = t < k, m1 = t + 8 < k;
                 const double amin = gmin(fmin(m0 ? t0v : INFINITY, m1 ? t1v : INFINITY));
@@ -505,13 +510,13 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                         if (m1 && !keep1) state[i1] = (i1 == last_added && alpha == 0.0) ? 2 : 0;
                         const int k0r = __popc(bk0 & ((1u << t) - 1u));
                         const int k1r = __popc(bk0) + __popc(bk1 & ((1u << t) - 1u));
-                        const double rs = rcp_d(ssum > 0.0 ? ssum : 1.0);
+                        const double rs = cons ? rcp_d(ssum > 0.0 ? ssum : 1.0) : 1.0;
                         if (keep0) { idx[k0r] = i0; aFs[k0r] = n0v * rs; }
                         if (keep1) { idx[k1r] = i1; aFs[k1r] = n1v * rs; }
                         k = __popc(bk0) + __popc(bk1);
                         last_added = -1;
                         ++pivots;
-                        if (k == 0 || pivots > max_pivots) { st = 2; fell = true; }
+                        if ((k == 0 && cons) || pivots > max_pivots) { st = 2; fell = true; }
                     }
                     __syncwarp();
                     if (ratio) {
@@ -537,7 +542,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 const int kw2 = wmax(resid_due ? k : 0);
                 {
                     float h0[16], h1[16];
-                    const double rs = rcp_d(accepted ? sq : 1.0);
+                    const double rs = cons ? rcp_d(accepted ? sq : 1.0) : 0.0;      // pos: H = K, no projection
                     const double u0 = q0 * rs, u1 = q1 * rs;
 #pragma unroll
                     for (int c2 = 0; c2 < 8; ++c2) {
@@ -621,7 +626,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 *reinterpret_cast<float4 *>(gs + 4 * t) = g4;
                 __syncwarp();
                 float nu = 0.0f;
-                if (accepted) {
+                if (accepted && cons) {
                     if (t < k) nu += gs[i0] * (float)a0;
                     if (t + 8 < k) nu += gs[i1] * (float)a1;
                 }
@@ -698,7 +703,7 @@ finish_sweep_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ cou
                 sbad |= !(sv[c].x > 0.0f) || !isfinite(sv[c].x) || !(sv[c].y > 0.0f) || !isfinite(sv[c].y);
             sbad = ((__ballot_sync(FULL, sbad) >> (8 * g)) & 0xffu) != 0u;
             if (wr && sbad) info |= LINMIN_INFO_BAD_SIGMA;
-            const bool doj = (st == 1) && !sbad && k > 1;
+            const bool doj = (st == 1) && !sbad && k > (cons ? 1 : 0);
             const int kj = wmax(doj ? k : 0);
             if (wr) { sgs[t] = 0.0f; sgs[t + 8] = 0.0f; }
             for (int ib = 0; ib < kj; ib += IT) {

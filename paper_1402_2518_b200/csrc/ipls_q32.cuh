@@ -140,6 +140,7 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
     // ---- per-lane state of my pixel: rows t + 4 s
     float a[S], lam[S], gmb[S];          // gmb = G a - b
     float nu = 0.0f, sc = 1.0f, lam0 = 1.0f;
+    const float consf = lib.cons ? 1.0f : 0.0f;
     int flags = 0, iters = 0, pix = -1;
     bool done = true;                    // "needs a pixel"
     bool idle = false;                   // no pixel left for this group
@@ -159,7 +160,7 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
                 gp = fmaf(a[s], lam[s], gp);
             }
             rdm = gmax(rdm); sa = gsum(sa); gp = gsum(gp);
-            rp = sa - 1.0f;
+            rp = consf * (sa - 1.0f);
             mu = gp * (1.0f / 32.0f);
             if (!done && !idle) {
                 if (flags & LINMIN_INFO_NONFINITE_INPUT) {
@@ -364,7 +365,7 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
             swz = fmaf(zd, rr[s].y, swz);
         }
         sww = gsum(sww); swz = gsum(swz);
-        const float rsww = rcp_approx(sww);
+        const float rsww = consf * rcp_approx(sww);       // pos: no equality constraint, dnu == 0 (nu stays 0)
         float dnu = (swz + rp) * rsww;
         float da[S];
 #pragma unroll

@@ -43,6 +43,7 @@ struct linmin_library {
     int sm_count = 0;
     cudaStream_t stream = nullptr;   // stream the handle was created on (frees are ordered on it)
     float *A = nullptr, *At = nullptr, *Ac = nullptr, *c = nullptr, *Gc = nullptr, *Gi = nullptr, *Giq = nullptr;
+    linmin_library *pos_twin = nullptr;   // slo at R = 32: the same library under positivity only (launch_solve)
     float *Gpad = nullptr;           // more than 64 endmembers: Gc zero-padded to whole 32 x 32 blocks (ipls_c256.cuh)
     float *scal = nullptr;           // device scalars: gdmax, sum of Giq
     int *flags = nullptr;            // device word: bit 0 = non-finite library
@@ -199,8 +200,9 @@ void note_use(const linmin_library *lib, cudaStream_t stream) {
     if (cudaEventRecord(lib->use_event[slot], stream) != cudaSuccess) { (void)cudaGetLastError(); lib->use_overflow = true; }
 }
 
-int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
-                 const Resolved &o, float *coeffs, float *csig, float *resid) {
+// prewhitened: Y is already Y W' (the caller did the renormalisation of this handle's covariance)
+int solve_core(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
+               const Resolved &o, float *coeffs, float *csig, float *resid, bool prewhitened) {
     const int L = lib->L, R = lib->Ri;      // R: the endmembers the kernels see (slack included)
     const bool cons = lib->constraint != LINMIN_CONSTRAINT_POSITIVITY_ONLY;
     LibView lv = view_of(lib);
@@ -211,7 +213,7 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     // ---- renormalised problem (eq. 6): Y' = Y W' into a workspace, then the unweighted path on
     //      (A', Y') with unit noise
     float *Yw = nullptr;
-    if (lib->weighting != LINMIN_WEIGHTING_NONE) {
+    if (lib->weighting != LINMIN_WEIGHTING_NONE && !prewhitened) {
         CK(staging_alloc((void **)&Yw, (size_t)N * L * sizeof(float), o.stream));
         CK(launch_whiten_spectra(Y, o.ldY, N, L, lib->W, lib->weighting == LINMIN_WEIGHTING_SHARED_DIAGONAL, Yw,
                                  lib->sm_count, o.stream));
@@ -233,12 +235,16 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     prm.has_sigma = sigma != nullptr;
     prm.max_iter = o.max_iter; prm.gap_tol = o.gap_tol; prm.feas_tol = o.feas_tol;
     prm.coeffs = coeffs; prm.coeff_sigma = csig; prm.resid = resid; prm.info = o.info;
+    // pos: the library is not centred, so the projections b = A'y that set the stopping scale are two orders of magnitude
+    // above the gradients that decide the support; with the sto thresholds IPLS handed over supports that needed 1.9
+    // repairs per pixel in the finish (0.24 with these; config-4 data: finish 36 -> 11 ms per 2^20 pixels, IPLS 6.2 -> 7.6)
+    if (!cons) { prm.gap_tol *= 0.01f; prm.feas_tol *= 0.01f; }
 
     // ---- K1: projection + IPLS
     // per-call workspace, because one handle may serve several streams: the work counters of the persistent
     // kernels (8 words), then two pixel lists of finish_sweep (count + one entry per pixel each): the overflow
     // list (supports above 16) and the repair list (pixels whose support changes after the first round)
-    const bool use_f8 = cons && finish_sweep_supported(L, R);
+    const bool use_f8 = finish_sweep_supported(L, R);
     unsigned int *ws = nullptr;
     const size_t ws_words = 8 + (use_f8 ? 2 * ((size_t)N + 1) : 0);
     CK(staging_alloc((void **)&ws, ws_words * sizeof(unsigned int), o.stream));
@@ -246,7 +252,7 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     CK(cudaMemsetAsync(ws, 0, std::min<size_t>(9, ws_words) * sizeof(unsigned int), o.stream));
     unsigned int *counters = ws, *overflow = ws + 8, *repair = ws + 8 + ((size_t)N + 1);
     if (use_f8) CK(cudaMemsetAsync(repair, 0, sizeof(unsigned int), o.stream));
-    if (cons && R == 32 && start_r32_warps(L) > 0) {
+    if (R == 32 && start_r32_warps(L) > 0) {
         // K0 (projection + start point, one record per pixel) and K1 (the iteration), in chunks of 2^21 pixels
         // so that the record workspace stays at 0.8 GB whatever N is
         const int64_t chunk = (int64_t)1 << 21;
@@ -291,20 +297,7 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     }
     if (lib->timing) CK(cudaEventRecord(lib->ev[1], o.stream));
     // ---- K2: exact finish + uncertainty + residual
-    if (use_f8) {
-        // first round for every pixel (91 % end there), then the others, packed, to their end: a warp's four
-        // pixels share every round, so a repair in the main pass would stall the three that are done
-        CK(launch_finish_sweep_tu(lv, prm, lib->sm_count, counters + 1, overflow, nullptr, repair, o.stream));
-        ++launches;
-        CK(launch_finish_sweep_tu(lv, prm, lib->sm_count, counters + 3, overflow, repair, nullptr, o.stream));
-        ++launches;
-        // pixels whose support outgrew finish_sweep (none on the synthetic cubes): one-warp-per-pixel kernel
-        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, o.stream));
-        ++launches;
-    } else if (cons && finish_fast_supported(L, R)) {
-        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, nullptr, o.stream));
-        ++launches;
-    } else {
+    auto launch_finish_any = [&](const unsigned int *list) -> int {      // one warp per pixel, any size, any constraint
         const int KMAX = R <= 32 ? R : 64;
         size_t per_warp = (finish_warp_bytes(L, R, KMAX) + 15) & ~(size_t)15;
         int warps = (int)std::min<size_t>(8, (200 * 1024) / per_warp);
@@ -312,9 +305,32 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
         size_t smem = per_warp * warps;
         CK(cudaFuncSetAttribute(finish_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int grid = persistent_grid(finish_kernel, warps * 32, smem, lib->sm_count, N, warps);
-        finish_kernel<<<grid, warps * 32, smem, o.stream>>>(lv, prm, KMAX);
+        finish_kernel<<<grid, warps * 32, smem, o.stream>>>(lv, prm, KMAX, list);
         CK(cudaGetLastError());
         ++launches;
+        return LINMIN_OK;
+    };
+    if (use_f8) {
+        // first round for every pixel (91 % end there), then the others, packed, to their end: a warp's four
+        // pixels share every round, so a repair in the main pass would stall the three that are done
+        CK(launch_finish_sweep_tu(lv, prm, lib->sm_count, counters + 1, overflow, nullptr, repair, o.stream));
+        ++launches;
+        CK(launch_finish_sweep_tu(lv, prm, lib->sm_count, counters + 3, overflow, repair, nullptr, o.stream));
+        ++launches;
+        // pixels whose support outgrew finish_sweep (0.1 % on config 4): one-warp-per-pixel kernels
+        if (cons) {
+            CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, o.stream));
+            ++launches;
+        } else {
+            const int rc = launch_finish_any(overflow);
+            if (rc != LINMIN_OK) return rc;
+        }
+    } else if (cons && finish_fast_supported(L, R)) {
+        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, nullptr, o.stream));
+        ++launches;
+    } else {
+        const int rc = launch_finish_any(nullptr);
+        if (rc != LINMIN_OK) return rc;
     }
     if (R != lib->R) {
         const int grid = (int)std::min<int64_t>((N * lib->R + 255) / 256, (int64_t)lib->sm_count * 16);
@@ -328,6 +344,47 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     return LINMIN_OK;
 }
 
+// The solve of a handle.  slo at R = 32 has no slack endmember: two passes over the fast kernels, pos into a workspace
+// and sto into the caller's arrays, then the per-pixel choice (slo_select_kernel).
+int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
+                 const Resolved &o, float *coeffs, float *csig, float *resid) {
+    if (!lib->pos_twin) return solve_core(lib, Y, sigma, N, o, coeffs, csig, resid, false);
+    const int L = lib->L, R = lib->R;
+    struct FreeV { void *p; cudaStream_t s; ~FreeV() { if (p) cudaFreeAsync(p, s); } };
+    Resolved oc = o;
+    float *Yw = nullptr;
+    int extra = 0;
+    if (lib->weighting != LINMIN_WEIGHTING_NONE) {
+        CK(staging_alloc((void **)&Yw, (size_t)N * L * sizeof(float), o.stream));
+        CK(launch_whiten_spectra(Y, o.ldY, N, L, lib->W, lib->weighting == LINMIN_WEIGHTING_SHARED_DIAGONAL, Yw,
+                                 lib->sm_count, o.stream));
+        ++extra;
+        Y = Yw; sigma = nullptr; oc.ldY = L; oc.sstride = 0;
+    }
+    FreeV free_yw{Yw, o.stream};
+    float *cp = nullptr, *sp = nullptr, *rp = nullptr;
+    int32_t *ip = nullptr;
+    CK(staging_alloc((void **)&cp, (size_t)N * R * sizeof(float), o.stream));
+    FreeV f0{cp, o.stream};
+    if (csig) CK(staging_alloc((void **)&sp, (size_t)N * R * sizeof(float), o.stream));
+    FreeV f1{sp, o.stream};
+    if (resid) CK(staging_alloc((void **)&rp, (size_t)N * sizeof(float), o.stream));
+    FreeV f2{rp, o.stream};
+    if (o.info) CK(staging_alloc((void **)&ip, (size_t)N * sizeof(int32_t), o.stream));
+    FreeV f3{ip, o.stream};
+    Resolved op = oc;
+    op.info = ip;
+    int rc = solve_core(lib->pos_twin, Y, sigma, N, op, cp, sp, rp, true);
+    if (rc != LINMIN_OK) return rc;
+    rc = solve_core(lib, Y, sigma, N, oc, coeffs, csig, resid, true);
+    if (rc != LINMIN_OK) return rc;
+    const int grid = (int)std::min<int64_t>((N + 7) / 8, (int64_t)lib->sm_count * 16);
+    slo_select_kernel<<<grid, 256, 0, o.stream>>>(N, R, cp, sp, rp, ip, coeffs, csig, resid, o.info);
+    CK(cudaGetLastError());
+    lib->last_launches.store(lib->last_launches.load() + lib->pos_twin->last_launches.load() + extra + 1);
+    return LINMIN_OK;
+}
+
 // Once-per-library precompute, all of it on the device and enqueued on `stream`: copy of A,
 // centred library, transposed copy, Gram matrices, start-point data.  No host round trip; `wait_check` adds the
 // ONE synchronisation linmin_library_create documents (to return LINMIN_ERR_LIBRARY_NONFINITE).
@@ -335,7 +392,11 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
                         int constraint, int weighting, const float *cov, linmin_library **out) {
     *out = nullptr;
     if (weighting != LINMIN_WEIGHTING_NONE && !cov) return LINMIN_ERR_INVALID_ARGUMENT;
-    const int Ri = (constraint == LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE) ? R + 1 : R;
+    // slo: a slack endmember (sto on [A | 0]) -- except at R = 32, where the fast kernels exist for exactly
+    // 32 endmembers: there slo is the pos solution where its sum stays below one and the sto solution elsewhere
+    const bool twin = constraint == LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE && R == 32 && start_r32_warps(L) > 0 &&
+                      finish_sweep_supported(L, R);
+    const int Ri = (constraint == LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE && !twin) ? R + 1 : R;
     if (Ri > LINMIN_MAX_R) return LINMIN_ERR_UNSUPPORTED_SIZE;
     const bool cons = constraint != LINMIN_CONSTRAINT_POSITIVITY_ONLY;
     int dev = 0;
@@ -410,6 +471,11 @@ int library_create_impl(const float *A, int L, int R, cudaStream_t stream, bool 
     }
     cudaFreeAsync(Araw, stream); Araw = nullptr;
     if (covd) { cudaFreeAsync(covd, stream); covd = nullptr; }
+    if (twin) {     // (same A, same covariance: its non-finite / covariance flags are this handle's)
+        const int rc = library_create_impl(A, L, R, stream, on_host, false, LINMIN_CONSTRAINT_POSITIVITY_ONLY, weighting, cov,
+                                           &lib->pos_twin);
+        if (rc < 0) return fail(rc);
+    }
     if (wait_check) {
         int hflags = 0;
         CKF(cudaMemcpyAsync(&hflags, lib->flags, sizeof(int), cudaMemcpyDeviceToHost, stream));
@@ -474,6 +540,7 @@ void linmin_library_destroy(linmin_library *lib) {
         }
         lib->n_use = 0;
     }
+    if (lib->pos_twin) linmin_library_destroy(lib->pos_twin);      // (its frees go to the same stream, after the waits above)
     void *bufs[] = {lib->A, lib->At, lib->Ac, lib->c, lib->Gc, lib->Gi, lib->Giq, lib->scal, lib->G64, lib->W64, lib->flags,
                     lib->W, lib->Wd, lib->Cd, lib->Gpad};
     for (void *q : bufs) if (q) cudaFreeAsync(q, s);

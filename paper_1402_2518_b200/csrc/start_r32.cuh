@@ -64,7 +64,8 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
     __syncthreads();
     if (warp >= warps) return;
     const float gdmax = lib.scal[0];
-    const float rGiqTot = rcp_approx(lib.scal[1]);
+    const bool cons = lib.cons != 0;      // false: positivity only -- no nu, the start point is not normalised
+    const float rGiqTot = cons ? rcp_approx(lib.scal[1]) : 0.0f;
     const bool vec_ok = ((L & 3) == 0) && ((prm.ldY & 3) == 0) && ((reinterpret_cast<uintptr_t>(prm.Y) & 15) == 0);
     const int nchunks = Lp / CH;
 
@@ -203,7 +204,7 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
                 mnx.x = fminf(mnx.x, x2[r].x); mnx.y = fminf(mnx.y, x2[r].y);
                 mng.x = fminf(mng.x, g.x); mng.y = fminf(mng.y, g.y);
             }
-            float2 nu = make_float2(-gx.x, -gx.y);
+            float2 nu = cons ? make_float2(-gx.x, -gx.y) : make_float2(0.0f, 0.0f);
             const float2 dp = make_float2(fmaxf(-mnx.x, 0.0f), fmaxf(-mnx.y, 0.0f));
             const float2 dd = make_float2(fmaxf(-(mng.x + nu.x), 0.0f), fmaxf(-(mng.y + nu.y), 0.0f));
             float2 cl = make_float2(nu.x + dd.x, nu.y + dd.y);          // lambda = g + cl
@@ -230,7 +231,7 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
                 const float lsh = H_(cl) + dd2 + 1e-4f * sch;               // lambda = g + lsh
                 const float sa = H_(sxx) + 32.0f * (dp2 + 1e-3f);
                 float lam0 = H_(lmx) + dd2 + 1e-4f * sch;
-                const float rsa = 1.0f / sa;
+                const float rsa = cons ? 1.0f / sa : 1.0f;
                 float nuh = H_(nu);
                 const bool flat = !(lam0 > 0.0f) || !isfinite(lam0) || !isfinite(sa);      // degenerate data
                 if (flat) { lam0 = fmaxf(bmx, 1e-3f * gdmax); nuh = 0.0f; }
@@ -259,7 +260,7 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
                         }
                     const bool bd = h ? bad1 : bad0;
                     *reinterpret_cast<float4 *>(o + 96) = make_float4(nuh, sch, lam0, __int_as_float(bd ? LINMIN_INFO_NONFINITE_INPUT : 0));
-                    *reinterpret_cast<float4 *>(o + 100) = make_float4(gap * (1.0f / 32.0f), suma - 1.0f, 0.0f, 0.0f);
+                    *reinterpret_cast<float4 *>(o + 100) = make_float4(gap * (1.0f / 32.0f), cons ? suma - 1.0f : 0.0f, 0.0f, 0.0f);
                 }
 #undef H_
             }

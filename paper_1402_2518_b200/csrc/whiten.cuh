@@ -239,4 +239,30 @@ __global__ void strip_slack_kernel(const float *__restrict__ ci, const float *__
     }
 }
 
+// slo without a slack endmember (R = 32): the problem is convex, so its minimiser is the pos minimiser where that one has
+// sum a <= 1 and the sto minimiser elsewhere (the bound is active there).  One warp per pixel: where the pos result
+// qualifies it replaces the sto result already in the caller's arrays.
+__global__ void slo_select_kernel(int64_t N, int R, const float *__restrict__ cp, const float *__restrict__ sp,
+                                  const float *__restrict__ rp, const int32_t *__restrict__ ip,
+                                  float *__restrict__ coeffs, float *__restrict__ csig, float *__restrict__ resid,
+                                  int32_t *__restrict__ info) {
+    const int lane = threadIdx.x & 31;
+    const int64_t stride = (int64_t)gridDim.x * (blockDim.x >> 5);
+    for (int64_t p = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); p < N; p += stride) {
+        float s = 0.0f;
+        for (int r = lane; r < R; r += 32) s += cp[p * R + r];
+        s = warp_sum(s);
+        if (s <= 1.0f) {            // (a NaN sum, non-finite input, keeps the sto result: it is NaN as well)
+            for (int r = lane; r < R; r += 32) {
+                coeffs[p * R + r] = cp[p * R + r];
+                if (csig) csig[p * R + r] = sp[p * R + r];
+            }
+            if (lane == 0) {
+                if (resid) resid[p] = rp[p];
+                if (info) info[p] = ip[p];
+            }
+        }
+    }
+}
+
 }  // namespace linmin
