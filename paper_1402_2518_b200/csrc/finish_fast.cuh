@@ -73,6 +73,7 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
     if ((list && list[0] == 0u) || lib.flags[0]) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int L = lib.L, R = lib.R;
+    const bool cons = lib.cons != 0;      // false: positivity only (no normalisation, mu == nu == 0, H = K, empty support allowed)
     const int AST = ast(LV);
     double *G64s = (double *)smem_raw;                    // [R][R]
     float *At = (float *)(smem_raw + g64_bytes(R));        // [R][AST], zero padded beyond L (16 B aligned)
@@ -148,7 +149,7 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
             float ai = (lane < R) ? cout[lane] : -1.0f;
             bool in = ai > LINMIN_SUPPORT_THRESHOLD;
             unsigned m = __ballot_sync(FULL, in);
-            if (m == 0u) {   // can not happen for a point of the simplex; be safe: largest entry
+            if (m == 0u && cons) {   // can not happen for a point of the simplex; be safe: largest entry
                 float best = warp_max(ai);
                 m = __ballot_sync(FULL, ai == best);
                 m = m & (0u - m);
@@ -162,7 +163,7 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
             __syncwarp();
             if (lane < k) { myidx = idx[lane]; aF = aFs[lane]; }
             double s = warp_sum(aF);
-            aF /= s;
+            if (cons) aF /= s;
             if (lane < k) aFs[lane] = aF;
             __syncwarp();
         }
@@ -216,11 +217,11 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
                 k = __popc(km);
                 __syncwarp();
                 last_added = -1;
-                if (k == 0) { fallback = true; break; }
+                if (k == 0 && cons) { fallback = true; break; }
                 myidx = 0; aF = 0.0;
                 if (lane < k) { myidx = idx[lane]; aF = aFs[lane]; }
                 double s = warp_sum(aF);
-                aF /= s;
+                if (cons) aF /= s;
                 if (lane < k) aFs[lane] = aF;
                 __syncwarp();
                 if (++pivots > max_pivots) { fallback = true; break; }
@@ -279,7 +280,7 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
             sq = warp_sum(q);
             const double sp = warp_sum(x1);
             const double suma = warp_sum(aF);
-            const double mu = (sp - (1.0 - suma)) / sq;
+            const double mu = cons ? (sp - (1.0 - suma)) / sq : 0.0;
             const double atry = aF + x1 - mu * q;
             double amin = warp_min_d((lane < k) ? atry : INFINITY);
             if (!(amin > 0.0)) {
@@ -299,13 +300,13 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
                 int rank = __popc(km & lt_mask);
                 double s = warp_sum(keep ? an : 0.0);
                 __syncwarp();
-                if (keep) { idx[rank] = myidx; aFs[rank] = an / s; }
+                if (keep) { idx[rank] = myidx; aFs[rank] = cons ? an / s : an; }
                 k = __popc(km);
                 __syncwarp();
                 last_added = -1;
                 myidx = 0; aF = 0.0;
                 if (lane < k) { myidx = idx[lane]; aF = aFs[lane]; }
-                if (k == 0 || ++pivots > max_pivots) { fallback = true; break; }
+                if ((k == 0 && cons) || ++pivots > max_pivots) { fallback = true; break; }
                 continue;
             }
             // ---- accept; residual, nu and multipliers at the new point
@@ -352,7 +353,7 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
                 __syncwarp();
                 am = (lane < R) ? (float)tmp[lane] : 0.0f;
             }
-            const float nu = warp_sum(gi * am);
+            const float nu = cons ? warp_sum(gi * am) : 0.0f;
             float li = (st == 0) ? (nu - gi) : INFINITY;
             const float gmaxv = warp_max((lane < R) ? fabsf(gi) : 0.0f);
             const float lbest = warp_min(li);
@@ -424,7 +425,7 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
             float myout = 0.0f;                           // lane j < k: sigma of support member j
             if (sbad) {
                 info |= LINMIN_INFO_BAD_SIGMA;
-            } else if (k > 1 && !fallback) {
+            } else if (k > (cons ? 1 : 0) && !fallback) {
                 // W = L^-1 in place, columns from the last to the first (lane i owns row i)
                 for (int j = k - 1; j >= 0; --j) {
                     const int offj = j * k - (j * (j - 1)) / 2;
@@ -444,7 +445,7 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
                 }
                 // H = W'W - q q'/(1'q), symmetric, fp32; lane i fills row i (j <= i) and its mirror
                 {
-                    const double rs = 1.0 / sq;
+                    const double rs = cons ? 1.0 / sq : 0.0;        // pos: H = K, no projection
                     int offj = 0;
                     for (int j = 0; j < k; ++j) {
                         const double qj = shfl_d(q, j), dj = shfl_d(dinv, j);

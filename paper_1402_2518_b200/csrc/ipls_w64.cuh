@@ -95,7 +95,8 @@ ipls_w64_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
     if (warp >= warps) return;
 
     const float gdmax = lib.scal[0];
-    const float rGiqTot = 1.0f / lib.scal[1];
+    const bool cons = lib.cons != 0;      // false: positivity only -- no nu, the start point is not normalised
+    const float rGiqTot = cons ? 1.0f / lib.scal[1] : 0.0f;
     const float tau = 0.995f, fR = (float)R;
     const float pivot_floor = 1e-12f * gdmax;
     const bool va = t < R, vb = t + 32 < R;       // my rows exist
@@ -171,7 +172,7 @@ ipls_w64_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             const float gx = warp_sum(gra * xa + grb * xb);
             const float mnx = warp_min(fminf(va ? xa : INFINITY, vb ? xb : INFINITY));
             const float mng = warp_min(fminf(va ? gra : INFINITY, vb ? grb : INFINITY));
-            nu = -gx;
+            nu = cons ? -gx : 0.0f;
             const float dp = fmaxf(-mnx, 0.0f), dd = fmaxf(-(mng + nu), 0.0f);
             xa += dp; xb += dp; gra += nu + dd; grb += nu + dd;
             const float xlm = warp_sum((va ? xa * gra : 0.0f) + (vb ? xb * grb : 0.0f));
@@ -182,7 +183,7 @@ ipls_w64_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             la = gra + dd2 + 1e-4f * sc; lb = grb + dd2 + 1e-4f * sc;
             const float sa = warp_sum((va ? aa : 0.0f) + (vb ? ab : 0.0f));
             lam0 = warp_max(fmaxf(va ? la : 0.0f, vb ? lb : 0.0f));
-            const float rsa = 1.0f / sa;
+            const float rsa = cons ? 1.0f / sa : 1.0f;
             const bool ok = (lam0 > 0.0f) && isfinite(lam0) && isfinite(sa) && isfinite(rsa);
             if (ok) {
                 aa *= rsa; ab *= rsa;
@@ -204,7 +205,7 @@ ipls_w64_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             const float rdm = warp_max(fmaxf(va ? fabsf(wa - la) : 0.0f, vb ? fabsf(wbv - lb) : 0.0f));
             const float sa = warp_sum((va ? aa : 0.0f) + (vb ? ab : 0.0f));
             const float gp = warp_sum((va ? aa * la : 0.0f) + (vb ? ab * lb : 0.0f));
-            const float rp = sa - 1.0f;
+            const float rp = cons ? sa - 1.0f : 0.0f;
             if (gp <= prm.gap_tol * sc && rdm <= prm.feas_tol * sc && fabsf(rp) <= prm.feas_tol) { flags |= LINMIN_INFO_CONVERGED; break; }
             if (it >= prm.max_iter) { flags |= LINMIN_INFO_MAX_ITER; break; }
             ++iters;
@@ -313,7 +314,7 @@ ipls_w64_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter
             // ---- predictor
             float sww = warp_sum(rra.x * dinva * rra.x + rrb.x * dinvb * rrb.x);
             float swz = warp_sum(rra.x * dinva * rra.y + rrb.x * dinvb * rrb.y);
-            const float rsww = 1.0f / sww;
+            const float rsww = cons ? 1.0f / sww : 0.0f;       // pos: dnu == 0 (nu stays 0)
             float dnu = (swz + rp) * rsww;
             float xa = fmaf(-rra.x, dnu, rra.y) * dinva, xb = fmaf(-rrb.x, dnu, rrb.y) * dinvb;
             backward_sweep(tri, xa, xb, t);

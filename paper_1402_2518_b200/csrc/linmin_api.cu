@@ -270,7 +270,7 @@ int solve_core(const linmin_library *lib, const float *Y, const float *sigma, in
             CK(launch_ipls_q32(lv, prm, pb, pe, recbuf, lib->sm_count, tickets + c, o.stream));
             launches += 2;
         }
-    } else if (cons && R > 32 && R <= 64 && ipls_w64_warps(L) > 0) {
+    } else if (R > 32 && R <= 64 && ipls_w64_warps(L) > 0) {
         // 33..64 endmembers (CRISM-like config, the paper's 36 / 37 / 44 spectra): one warp per pixel, matrix in registers
         CK(launch_ipls_w64(lv, prm, lib->sm_count, counters, o.stream));
         ++launches;
@@ -318,14 +318,9 @@ int solve_core(const linmin_library *lib, const float *Y, const float *sigma, in
         CK(launch_finish_sweep_tu(lv, prm, lib->sm_count, counters + 3, overflow, repair, nullptr, o.stream));
         ++launches;
         // pixels whose support outgrew finish_sweep (0.1 % on config 4): one-warp-per-pixel kernels
-        if (cons) {
-            CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, o.stream));
-            ++launches;
-        } else {
-            const int rc = launch_finish_any(overflow);
-            if (rc != LINMIN_OK) return rc;
-        }
-    } else if (cons && finish_fast_supported(L, R)) {
+        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, o.stream));
+        ++launches;
+    } else if (finish_fast_supported(L, R)) {
         CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, nullptr, o.stream));
         ++launches;
     } else {
