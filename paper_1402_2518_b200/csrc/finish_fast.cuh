@@ -1,4 +1,4 @@
-// finish_fast.cuh -- exact finish + uncertainty + residual for R <= 32, L <= 512 (sm_100a).
+// finish_fast.cuh -- exact finish + uncertainty + residual for R <= 64 (supports up to 32 members), L <= 512 (sm_100a).
 //
 // Same mathematics as finish.cuh (read its header: PAPER.md:54-68 optimality conditions,
 // PAPER.md:88 uncertainty reading R3, PAPER.md:143 RMS reading R8), re-mapped for speed:
@@ -27,10 +27,10 @@ __host__ __device__ inline size_t g64_bytes(int R) { return ((size_t)R * R * 8 +
 __host__ __device__ inline size_t cta_bytes(int R, int LV) { return g64_bytes(R) + (size_t)R * ast(LV) * 4; }
 __host__ __device__ inline size_t warp_bytes(int LV) {
     return (size_t)(KM * (KM + 1) / 2) * 8   // Lf
-           + (size_t)2 * KM * 8              // aFs, tmp
+           + (size_t)KM * 8 + 64 * 8         // aFs, tmp (by endmember: up to 64)
            + (size_t)KM * KM * 4             // Hs
            + (size_t)128 * LV * 4            // rbuf
-           + (size_t)KM * 4 + KM;            // idx, state
+           + (size_t)KM * 4 + 64;            // idx, state (by endmember)
 }
 
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(FULL, v, src); }
@@ -65,10 +65,14 @@ __device__ __forceinline__ float reduce4(float v0, float v1, float v2, float v3,
 
 }  // namespace ff
 
-template <int LV>
+// RH = 1: R <= 32, lane i owns endmember i; RH = 2: R <= 64, lane i owns endmembers i and i + 32.  The support is capped
+// at KM = 32 members either way; with RH = 2 a pixel that needs more goes to `overflow` ([0] = count, [1 + i] = pixel)
+// untouched and is finished by the any-size kernel.
+template <int LV, int RH>
 __global__ void __launch_bounds__(512, 1)
 finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ counter,
-                   const unsigned int *__restrict__ list /* NULL: all pixels; else [0] = count, [1 + i] = pixel */) {
+                   const unsigned int *__restrict__ list /* NULL: all pixels; else [0] = count, [1 + i] = pixel */,
+                   unsigned int *__restrict__ overflow) {
     using namespace ff;
     if ((list && list[0] == 0u) || lib.flags[0]) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -82,10 +86,10 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
     double *Lf = (double *)wb;                             // packed lower, column-major, runtime k
     double *aFs = Lf + KM * (KM + 1) / 2;                  // [KM] coefficients on the support
     double *tmp = aFs + KM;                                // [KM]
-    float *Hs = (float *)(tmp + KM);                       // [KM][KM] symmetric
+    float *Hs = (float *)(tmp + 64);                       // [KM][KM] symmetric   (tmp: [64], by endmember)
     float *rbuf = Hs + KM * KM;                            // [128 LV] fp32 residual
     int *idx = (int *)(rbuf + 128 * LV);                   // [KM]
-    unsigned char *state = (unsigned char *)(idx + KM);    // [KM]: 0 free, 1 in F, 2 blocked
+    unsigned char *state = (unsigned char *)(idx + KM);    // [64] by endmember: 0 free, 1 in F, 2 blocked
 
     for (int e = threadIdx.x; e < R * R; e += blockDim.x) G64s[e] = lib.G64[e];
     for (int e = threadIdx.x; e < R * AST; e += blockDim.x) {
@@ -131,9 +135,13 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
             for (int q = 0; q < 4; ++q) bad |= !isfinite(yv[4 * v + q]);
         }
         if (__any_sync(FULL, bad)) {
-            if (lane < R) {
-                cout[lane] = qnan;
-                if (prm.coeff_sigma) prm.coeff_sigma[p * R + lane] = qnan;
+#pragma unroll
+            for (int h = 0; h < RH; ++h) {
+                const int e = lane + 32 * h;
+                if (e < R) {
+                    cout[e] = qnan;
+                    if (prm.coeff_sigma) prm.coeff_sigma[p * R + e] = qnan;
+                }
             }
             if (lane == 0) {
                 if (prm.resid) prm.resid[p] = qnan;
@@ -146,20 +154,34 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
         int myidx = 0;
         double aF = 0.0;
         {
-            float ai = (lane < R) ? cout[lane] : -1.0f;
-            bool in = ai > LINMIN_SUPPORT_THRESHOLD;
-            unsigned m = __ballot_sync(FULL, in);
-            if (m == 0u && cons) {   // can not happen for a point of the simplex; be safe: largest entry
-                float best = warp_max(ai);
-                m = __ballot_sync(FULL, ai == best);
-                m = m & (0u - m);
-                in = (m >> lane) & 1u;
-                ai = 1.0f;
+            float ai[RH];
+            bool in[RH];
+            unsigned m[2] = {0u, 0u};
+#pragma unroll
+            for (int h = 0; h < RH; ++h) {
+                ai[h] = (lane + 32 * h < R) ? cout[lane + 32 * h] : -1.0f;
+                in[h] = ai[h] > LINMIN_SUPPORT_THRESHOLD;
+                m[h] = __ballot_sync(FULL, in[h]);
             }
-            k = __popc(m);
-            int rank = __popc(m & lt_mask);
-            if (lane < R) state[lane] = in ? 1 : 0;
-            if (in) { idx[rank] = lane; aFs[rank] = (double)ai; }
+            if ((m[0] | m[1]) == 0u && cons) {   // can not happen for a point of the simplex; be safe: largest entry
+                float best = warp_max(RH > 1 ? fmaxf(ai[0], ai[RH - 1]) : ai[0]);
+                m[0] = __ballot_sync(FULL, ai[0] == best);
+                m[0] = m[0] & (0u - m[0]);
+                if (RH > 1) { m[1] = m[0] ? 0u : __ballot_sync(FULL, ai[RH - 1] == best); m[1] = m[1] & (0u - m[1]); }
+#pragma unroll
+                for (int h = 0; h < RH; ++h) { in[h] = (m[h] >> lane) & 1u; ai[h] = 1.0f; }
+            }
+            k = __popc(m[0]) + __popc(m[1]);
+            if (RH > 1 && k > KM) {          // wider than this kernel's cap: the any-size kernel takes the pixel as it is
+                if (lane == 0 && overflow) { const unsigned slot = atomicAdd(overflow, 1u); overflow[1 + slot] = (unsigned)p; }
+                continue;
+            }
+#pragma unroll
+            for (int h = 0; h < RH; ++h) {
+                const int rank = (h ? __popc(m[0]) : 0) + __popc(m[h] & lt_mask);
+                if (lane + 32 * h < R) state[lane + 32 * h] = in[h] ? 1 : 0;
+                if (in[h]) { idx[rank] = lane + 32 * h; aFs[rank] = (double)ai[h]; }
+            }
             __syncwarp();
             if (lane < k) { myidx = idx[lane]; aF = aFs[lane]; }
             double s = warp_sum(aF);
@@ -331,49 +353,70 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
                     make_float4((float)r[4 * v + 0], (float)r[4 * v + 1], (float)r[4 * v + 2], (float)r[4 * v + 3]);
             __syncwarp();
             // g_i = A_i' r for every endmember (fp32 dot products of the fp64 residual); lane i
-            float gi = 0.0f;
-            {
-                const float *row = At + (lane < R ? lane : 0) * AST;
+            float gi[RH];
+#pragma unroll
+            for (int h = 0; h < RH; ++h) {
+                const float *row = At + (lane + 32 * h < R ? lane + 32 * h : 0) * AST;
+                float g = 0.0f;
 #pragma unroll 8
                 for (int c = 0; c < 32 * LV; ++c) {
                     float4 a4 = *reinterpret_cast<const float4 *>(row + 4 * c);
                     float4 r4 = *reinterpret_cast<const float4 *>(rbuf + 4 * c);
-                    gi = fmaf(a4.x, r4.x, gi); gi = fmaf(a4.y, r4.y, gi);
-                    gi = fmaf(a4.z, r4.z, gi); gi = fmaf(a4.w, r4.w, gi);
+                    g = fmaf(a4.x, r4.x, g); g = fmaf(a4.y, r4.y, g);
+                    g = fmaf(a4.z, r4.z, g); g = fmaf(a4.w, r4.w, g);
                 }
+                gi[h] = g;
             }
             // nu = sum_{j in F} g_j a_j : bring a_F to endmember lanes through state/aFs
-            float am = 0.0f;
-            const int st = (lane < R) ? state[lane] : 2;
+            int st[RH];
+            float nus = 0.0f, gab = 0.0f;
             {
                 // lane j < k holds (myidx, aF); scatter a_F to endmember order via shared memory
-                if (lane < R) tmp[lane] = 0.0;
+#pragma unroll
+                for (int h = 0; h < RH; ++h) if (lane + 32 * h < R) tmp[lane + 32 * h] = 0.0;
                 __syncwarp();
                 if (lane < k) tmp[myidx] = aF;
                 __syncwarp();
-                am = (lane < R) ? (float)tmp[lane] : 0.0f;
+#pragma unroll
+                for (int h = 0; h < RH; ++h) {
+                    const bool live = lane + 32 * h < R;
+                    st[h] = live ? state[lane + 32 * h] : 2;
+                    nus = fmaf(gi[h], live ? (float)tmp[lane + 32 * h] : 0.0f, nus);
+                    gab = fmaxf(gab, live ? fabsf(gi[h]) : 0.0f);
+                }
             }
-            const float nu = cons ? warp_sum(gi * am) : 0.0f;
-            float li = (st == 0) ? (nu - gi) : INFINITY;
-            const float gmaxv = warp_max((lane < R) ? fabsf(gi) : 0.0f);
-            const float lbest = warp_min(li);
-            unsigned mm = __ballot_sync(FULL, li == lbest && st == 0);
-            if (!(lbest < -1e-6f * gmaxv) || mm == 0u) break;          // optimal
+            const float nu = cons ? warp_sum(nus) : 0.0f;
+            float li[RH], lmin = INFINITY;
+#pragma unroll
+            for (int h = 0; h < RH; ++h) { li[h] = (st[h] == 0) ? (nu - gi[h]) : INFINITY; lmin = fminf(lmin, li[h]); }
+            const float gmaxv = warp_max(gab);
+            const float lbest = warp_min(lmin);
+            unsigned mm[2] = {0u, 0u};
+#pragma unroll
+            for (int h = 0; h < RH; ++h) mm[h] = __ballot_sync(FULL, li[h] == lbest && st[h] == 0);
+            if (!(lbest < -1e-6f * gmaxv) || (mm[0] | mm[1]) == 0u) break;          // optimal
             if (k >= KM || pivots >= max_pivots) { fallback = true; break; }
-            const int jadd = __ffs(mm) - 1;
-            if (lane == jadd) state[jadd] = 1;
+            const int jadd = mm[0] ? (__ffs(mm[0]) - 1) : (32 + __ffs(mm[1]) - 1);
+            if (lane == (jadd & 31)) state[jadd] = 1;
             if (lane == k) { myidx = jadd; aF = 0.0; idx[k] = jadd; aFs[k] = 0.0; }
             ++k; ++pivots; last_added = jadd;
             __syncwarp();
         }
 
         // ---- outputs: coefficients (exact zeros off the support)
+        if (RH > 1 && fallback && k >= KM && overflow) {    // the support wants to outgrow the cap: any-size kernel
+            if (lane == 0) { const unsigned slot = atomicAdd(overflow, 1u); overflow[1 + slot] = (unsigned)p; }
+            __syncwarp();
+            continue;
+        }
         {
-            if (lane < R) tmp[lane] = 0.0;
+#pragma unroll
+            for (int h = 0; h < RH; ++h) if (lane + 32 * h < R) tmp[lane + 32 * h] = 0.0;
             __syncwarp();
             if (lane < k) tmp[myidx] = aF;
             __syncwarp();
-            if (lane < R) cout[lane] = (float)tmp[lane];
+#pragma unroll
+            for (int h = 0; h < RH; ++h) if (lane + 32 * h < R) cout[lane + 32 * h] = (float)tmp[lane + 32 * h];
         }
         if (fallback) {
 #pragma unroll
@@ -505,11 +548,13 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
                 }
             }
             // scatter to endmember order
-            if (lane < R) rbuf[lane] = 0.0f;
+#pragma unroll
+            for (int h = 0; h < RH; ++h) if (lane + 32 * h < R) rbuf[lane + 32 * h] = 0.0f;
             __syncwarp();
             if (lane < k) rbuf[myidx] = myout;
             __syncwarp();
-            if (lane < R) sout[lane] = sbad ? qnan : rbuf[lane];
+#pragma unroll
+            for (int h = 0; h < RH; ++h) if (lane + 32 * h < R) sout[lane + 32 * h] = sbad ? qnan : rbuf[lane + 32 * h];
         }
         if (prm.info && lane == 0) {
             int pv = pivots > 255 ? 255 : pivots;
@@ -519,34 +564,47 @@ finish_fast_kernel(LibView lib, SolveParams prm, unsigned int *__restrict__ coun
     }
 }
 
-inline bool finish_fast_supported(int L, int R) { return R <= 32 && L <= 512; }
+inline bool finish_fast_supported(int L, int R) { return R <= 64 && L <= 512; }
 
 inline int finish_fast_lv(int L) { return L <= 128 ? 1 : (L <= 256 ? 2 : 4); }
 
-template <int LV>
-inline cudaError_t launch_finish_fast_lv(const LibView &lv, const SolveParams &prm, int sm_count,
-                                         unsigned int *counter, const unsigned int *list, cudaStream_t stream) {
+template <int LV, int RH>
+inline cudaError_t launch_finish_fast_lv(const LibView &lv, const SolveParams &prm, int sm_count, unsigned int *counter,
+                                         const unsigned int *list, unsigned int *overflow, cudaStream_t stream) {
     const size_t cta = (ff::cta_bytes(lv.R, LV) + 15) & ~(size_t)15;
     const size_t per_warp = (ff::warp_bytes(LV) + 15) & ~(size_t)15;
+    if (cta + per_warp > 220 * 1024) return cudaErrorInvalidConfiguration;
     int warps = (int)std::min<size_t>(16, (220 * 1024 - cta) / per_warp);
-    if (warps < 1) return cudaErrorInvalidConfiguration;
     const size_t smem = cta + per_warp * warps;
-    cudaError_t e = cudaFuncSetAttribute(finish_fast_kernel<LV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(finish_fast_kernel<LV, RH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int64_t need = (prm.N + warps - 1) / warps;
     int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, sm_count));
-    finish_fast_kernel<LV><<<grid, warps * 32, smem, stream>>>(lv, prm, counter, list);
+    finish_fast_kernel<LV, RH><<<grid, warps * 32, smem, stream>>>(lv, prm, counter, list, overflow);
     return cudaGetLastError();
 }
 
-// counter must be zero (the caller clears it on the stream); list: see the kernel
-inline cudaError_t launch_finish_fast(const LibView &lv, const SolveParams &prm, int sm_count,
-                                      unsigned int *counter, const unsigned int *list, cudaStream_t stream) {
-    switch (finish_fast_lv(lv.L)) {
-        case 1: return launch_finish_fast_lv<1>(lv, prm, sm_count, counter, list, stream);
-        case 2: return launch_finish_fast_lv<2>(lv, prm, sm_count, counter, list, stream);
-        default: return launch_finish_fast_lv<4>(lv, prm, sm_count, counter, list, stream);
+// counter (and overflow[0], when given) must be zero (the caller clears them on the stream); list, overflow: see the kernel
+inline cudaError_t launch_finish_fast(const LibView &lv, const SolveParams &prm, int sm_count, unsigned int *counter,
+                                      const unsigned int *list, unsigned int *overflow, cudaStream_t stream) {
+    if (lv.R <= 32) {
+        switch (finish_fast_lv(lv.L)) {
+            case 1: return launch_finish_fast_lv<1, 1>(lv, prm, sm_count, counter, list, overflow, stream);
+            case 2: return launch_finish_fast_lv<2, 1>(lv, prm, sm_count, counter, list, overflow, stream);
+            default: return launch_finish_fast_lv<4, 1>(lv, prm, sm_count, counter, list, overflow, stream);
+        }
     }
+    switch (finish_fast_lv(lv.L)) {
+        case 1: return launch_finish_fast_lv<1, 2>(lv, prm, sm_count, counter, list, overflow, stream);
+        case 2: return launch_finish_fast_lv<2, 2>(lv, prm, sm_count, counter, list, overflow, stream);
+        default: return launch_finish_fast_lv<4, 2>(lv, prm, sm_count, counter, list, overflow, stream);
+    }
+}
+// fits in shared memory with at least four warps?
+inline bool finish_fast_fits(int L, int R) {
+    const int LV = finish_fast_lv(L);
+    const size_t cta = (ff::cta_bytes(R, LV) + 15) & ~(size_t)15, per_warp = (ff::warp_bytes(LV) + 15) & ~(size_t)15;
+    return finish_fast_supported(L, R) && cta + 4 * per_warp <= 220 * 1024;
 }
 
 }  // namespace linmin

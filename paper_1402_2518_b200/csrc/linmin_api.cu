@@ -245,8 +245,9 @@ int solve_core(const linmin_library *lib, const float *Y, const float *sigma, in
     // kernels (8 words), then two pixel lists of finish_sweep (count + one entry per pixel each): the overflow
     // list (supports above 16) and the repair list (pixels whose support changes after the first round)
     const bool use_f8 = finish_sweep_supported(L, R);
+    const bool use_ff64 = !use_f8 && R > 32 && finish_fast_fits(L, R);      // 33..64 endmembers: finish_fast + its overflow list
     unsigned int *ws = nullptr;
-    const size_t ws_words = 8 + (use_f8 ? 2 * ((size_t)N + 1) : 0);
+    const size_t ws_words = 8 + (use_f8 ? 2 * ((size_t)N + 1) : (use_ff64 ? (size_t)N + 1 : 0));
     CK(staging_alloc((void **)&ws, ws_words * sizeof(unsigned int), o.stream));
     struct Free { unsigned int *p; cudaStream_t s; ~Free() { cudaFreeAsync(p, s); } } free_ws{ws, o.stream};
     CK(cudaMemsetAsync(ws, 0, std::min<size_t>(9, ws_words) * sizeof(unsigned int), o.stream));
@@ -318,10 +319,16 @@ int solve_core(const linmin_library *lib, const float *Y, const float *sigma, in
         CK(launch_finish_sweep_tu(lv, prm, lib->sm_count, counters + 3, overflow, repair, nullptr, o.stream));
         ++launches;
         // pixels whose support outgrew finish_sweep (0.1 % on config 4): one-warp-per-pixel kernels
-        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, o.stream));
+        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, overflow, nullptr, o.stream));
         ++launches;
-    } else if (finish_fast_supported(L, R)) {
-        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, nullptr, o.stream));
+    } else if (use_ff64) {
+        // one warp per pixel, two endmembers per lane, supports up to 32; wider ones go on to the any-size kernel
+        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, nullptr, overflow, o.stream));
+        ++launches;
+        const int rc = launch_finish_any(overflow);
+        if (rc != LINMIN_OK) return rc;
+    } else if (R <= 32 && finish_fast_fits(L, R)) {
+        CK(launch_finish_fast(lv, prm, lib->sm_count, counters + 2, nullptr, nullptr, o.stream));
         ++launches;
     } else {
         const int rc = launch_finish_any(nullptr);
