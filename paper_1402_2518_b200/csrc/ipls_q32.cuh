@@ -82,6 +82,9 @@ __device__ __forceinline__ void backward_subst(const float2 (&m2)[S][2 * S], con
 
 // counter: device word, zero (the caller clears it on the stream before the launch); rec: records of K0 for the
 // pixels [p_begin, p_end).
+// CONS false: positivity only (no equality constraint: r_p == 0, dnu == 0, nu stays 0).  A template parameter, not a flag:
+// the flag cost the sto path 1.6 % (one more multiply on the chain through dnu).
+template <bool CONS>
 __global__ void __launch_bounds__(q32::WARPS * 32, 1)
 ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, const float *__restrict__ rec,
                 unsigned int *__restrict__ counter) {
@@ -140,7 +143,6 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
     // ---- per-lane state of my pixel: rows t + 4 s
     float a[S], lam[S], gmb[S];          // gmb = G a - b
     float nu = 0.0f, sc = 1.0f, lam0 = 1.0f;
-    const float consf = lib.cons ? 1.0f : 0.0f;
     int flags = 0, iters = 0, pix = -1;
     bool done = true;                    // "needs a pixel"
     bool idle = false;                   // no pixel left for this group
@@ -160,7 +162,7 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
                 gp = fmaf(a[s], lam[s], gp);
             }
             rdm = gmax(rdm); sa = gsum(sa); gp = gsum(gp);
-            rp = consf * (sa - 1.0f);
+            rp = CONS ? sa - 1.0f : 0.0f;
             mu = gp * (1.0f / 32.0f);
             if (!done && !idle) {
                 if (flags & LINMIN_INFO_NONFINITE_INPUT) {
@@ -365,7 +367,7 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
             swz = fmaf(zd, rr[s].y, swz);
         }
         sww = gsum(sww); swz = gsum(swz);
-        const float rsww = consf * rcp_approx(sww);       // pos: no equality constraint, dnu == 0 (nu stays 0)
+        const float rsww = CONS ? rcp_approx(sww) : 0.0f;
         float dnu = (swz + rp) * rsww;
         float da[S];
 #pragma unroll
@@ -440,12 +442,14 @@ ipls_q32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, co
 inline cudaError_t launch_ipls_q32(const LibView &lv, const SolveParams &prm, int64_t p_begin, int64_t p_end,
                                    const float *rec, int sm_count, unsigned int *counter, cudaStream_t stream) {
     const size_t smem = q32::smem_floats() * sizeof(float);
-    cudaError_t e = cudaFuncSetAttribute(ipls_q32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = lv.cons ? cudaFuncSetAttribute(ipls_q32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                            : cudaFuncSetAttribute(ipls_q32_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int64_t n = p_end - p_begin;
     const int64_t need = (n + 8 * q32::WARPS - 1) / (8 * q32::WARPS);
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, (int64_t)sm_count));
-    ipls_q32_kernel<<<grid, q32::WARPS * 32, smem, stream>>>(lv, prm, p_begin, p_end, rec, counter);
+    if (lv.cons) ipls_q32_kernel<true><<<grid, q32::WARPS * 32, smem, stream>>>(lv, prm, p_begin, p_end, rec, counter);
+    else ipls_q32_kernel<false><<<grid, q32::WARPS * 32, smem, stream>>>(lv, prm, p_begin, p_end, rec, counter);
     return cudaGetLastError();
 }
 

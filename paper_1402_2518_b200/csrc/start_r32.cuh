@@ -36,6 +36,8 @@ __host__ __device__ inline size_t warp_floats() { return (size_t)2 * TP * YST; }
 }  // namespace s32
 
 // rec: N x REC floats (workspace).  One warp per tile of 128 pixels, static partition (the work per pixel is fixed).
+// CONS false: positivity only -- no nu, the start point is not normalised
+template <bool CONS>
 __global__ void __launch_bounds__(s32::WARPS * 32, 1)
 start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, float *__restrict__ rec, int warps) {
     using namespace s32;
@@ -64,7 +66,7 @@ start_r32_kernel(LibView lib, SolveParams prm, int64_t p_begin, int64_t p_end, f
     __syncthreads();
     if (warp >= warps) return;
     const float gdmax = lib.scal[0];
-    const bool cons = lib.cons != 0;      // false: positivity only -- no nu, the start point is not normalised
+    constexpr bool cons = CONS;
     const float rGiqTot = cons ? rcp_approx(lib.scal[1]) : 0.0f;
     const bool vec_ok = ((L & 3) == 0) && ((prm.ldY & 3) == 0) && ((reinterpret_cast<uintptr_t>(prm.Y) & 15) == 0);
     const int nchunks = Lp / CH;
@@ -283,11 +285,13 @@ inline cudaError_t launch_start_r32(const LibView &lv, const SolveParams &prm, i
     const int warps = start_r32_warps(lv.L);
     if (warps < 1) return cudaErrorInvalidConfiguration;
     const size_t smem = start_r32_smem(lv.L, warps);
-    cudaError_t e = cudaFuncSetAttribute(start_r32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = lv.cons ? cudaFuncSetAttribute(start_r32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                            : cudaFuncSetAttribute(start_r32_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int64_t tiles = (p_end - p_begin + s32::TP - 1) / s32::TP;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((tiles + warps - 1) / warps, sm_count));
-    start_r32_kernel<<<grid, s32::WARPS * 32, smem, stream>>>(lv, prm, p_begin, p_end, rec, warps);
+    if (lv.cons) start_r32_kernel<true><<<grid, s32::WARPS * 32, smem, stream>>>(lv, prm, p_begin, p_end, rec, warps);
+    else start_r32_kernel<false><<<grid, s32::WARPS * 32, smem, stream>>>(lv, prm, p_begin, p_end, rec, warps);
     return cudaGetLastError();
 }
 
