@@ -71,6 +71,8 @@ extern "C" {
 #define LINMIN_ERR_OUT_OF_MEMORY (-5)
 #define LINMIN_ERR_LIBRARY_NONFINITE (-6) /* A contains NaN or Inf */
 #define LINMIN_ERR_COVARIANCE (-7)        /* the noise covariance is not finite / not positive definite */
+#define LINMIN_ERR_STATIC_SCRATCH (-8)    /* linmin_detection_thresholds_static only: R > LINMIN_STATIC_MAX_R, the
+                                             library's fixed scratch array has no room for that many endmembers */
 #define LINMIN_WARN_RANK_DEFICIENT 1      /* R > L: minimiser may be non-unique (PAPER.md:92 asks R <= L) */
 
 #define LINMIN_MAX_R 256
@@ -200,6 +202,28 @@ int linmin_additional_spectra(const float *wavelength, int32_t L, int32_t n_extr
  * thresholds_out: R floats.  Sums in fp64 in a fixed order (results do not depend on scheduling). */
 int linmin_detection_thresholds(const float *coeffs, const unsigned char *present, int64_t N, int32_t R,
                                 float *thresholds_out, void *stream);
+
+/* The same thresholds for callers that cannot let the library allocate device memory: an application that gave the
+ * whole GPU to its own arena at start-up (an allocation made here would fail or take memory it has planned for),
+ * or a latency-bound loop that cannot afford the device-wide synchronisation and unbounded duration an allocation
+ * may cost.  linmin_detection_thresholds draws its per-block partial sums from the library's staging pool; this
+ * call keeps them in ONE fixed array inside the library image and calls no cudaMalloc / cudaFree, no pool and no
+ * other allocating routine.  Inputs and outputs are the caller's, as above.
+ *   Limit: R <= LINMIN_STATIC_MAX_R (else LINMIN_ERR_STATIC_SCRATCH; nothing is launched); N is not limited (at most
+ *     LINMIN_STATIC_MAX_BLOCKS thread blocks walk the data).  The array takes LINMIN_STATIC_MAX_BLOCKS x
+ *     LINMIN_STATIC_MAX_R x 6 doubles = 384 KiB on every GPU that loads the library, until the process exits.
+ *   First call on a device: looks the array's address on that device up (once, kept afterwards).  Make that first
+ *     call during set-up, before any stream capture is begun.
+ *   Sharing: every call on a device uses the same array, which still holds the previous call's sums.  Nothing has
+ *     to be cleared (each call overwrites every slot it later reads), but two calls that overlap on the GPU -- on two
+ *     streams, or from two host threads -- race on it and return garbage: keep calls on one device in stream order.
+ *   Result: the blocks' fp64 sums are added in a fixed order, but the launch has fewer blocks than the pooled
+ *     call's, so the float32 thresholds equal linmin_detection_thresholds' to rounding (1 ulp), not always bit for
+ *     bit; repeated calls on the same data return the same bits. */
+#define LINMIN_STATIC_MAX_R 64
+#define LINMIN_STATIC_MAX_BLOCKS 128
+int linmin_detection_thresholds_static(const float *coeffs, const unsigned char *present, int64_t N, int32_t R,
+                                       float *thresholds_out, void *stream);
 
 /* The three detection conditions of PAPER.md:239-246: mask[p*R + i] = coeffs > thresholds[i] and coeff_sigma < coeffs
  * and resid[p] < rms_max ("10 times the dark current noise").  counts_out (optional): R detections per endmember. */

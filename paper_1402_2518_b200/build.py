@@ -13,7 +13,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblinmin.so")
 PROBE_LIB = os.path.join(HERE, "libfp32probe.so")     # bench-side helper (roofline denominator), not the product
 # source -> extra flags of its translation unit
-SOURCES = {"linmin_api.cu": [], "finish_sweep.cu": []}
+SOURCES = {"linmin_api.cu": [], "finish_sweep.cu": [], "thresholds_static.cu": []}
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false"]
 

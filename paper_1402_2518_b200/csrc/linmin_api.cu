@@ -513,6 +513,7 @@ const char *linmin_strerror(int code) {
         case LINMIN_ERR_OUT_OF_MEMORY: return "out of device memory";
         case LINMIN_ERR_LIBRARY_NONFINITE: return "library A contains a non-finite value";
         case LINMIN_ERR_COVARIANCE: return "noise covariance is not finite or not positive definite";
+        case LINMIN_ERR_STATIC_SCRATCH: return "more than 64 endmembers: beyond the fixed scratch array of linmin_detection_thresholds_static";
         case LINMIN_WARN_RANK_DEFICIENT: return "warning: R > L, the minimiser may be non-unique";
         default: return "unknown status code";
     }

@@ -22,6 +22,8 @@ ERR_CUDA = -4
 ERR_OUT_OF_MEMORY = -5
 ERR_LIBRARY_NONFINITE = -6
 ERR_COVARIANCE = -7
+ERR_STATIC_SCRATCH = -8
+STATIC_MAX_R = 64
 CONSTRAINT_SUM_TO_ONE, CONSTRAINT_SUM_LOWER_THAN_ONE, CONSTRAINT_POSITIVITY_ONLY = 0, 1, 2
 WEIGHTING_NONE, WEIGHTING_SHARED_COVARIANCE, WEIGHTING_SHARED_DIAGONAL = 0, 1, 2
 WARN_RANK_DEFICIENT = 1
@@ -38,7 +40,7 @@ EXPORTS = ["linmin_version", "linmin_strerror", "linmin_library_create", "linmin
            "linmin_library_last_launches", "linmin_library_enable_timing", "linmin_library_last_timing",
            "linmin_trim_memory",
            "linmin_unmix_lib", "linmin_unmix", "linmin_unmix_host",
-           "linmin_additional_spectra", "linmin_detection_thresholds", "linmin_detect", "linmin_second_pass",
+           "linmin_additional_spectra", "linmin_detection_thresholds", "linmin_detection_thresholds_static", "linmin_detect", "linmin_second_pass",
            "linmin_autofit"]
 
 
@@ -83,6 +85,7 @@ def load() -> ctypes.CDLL:
         lib.linmin_unmix_host.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_additional_spectra.argtypes = [P, I32, I32, P, I32, I32, P]
         lib.linmin_detection_thresholds.argtypes = [P, P, I64, I32, P, P]
+        lib.linmin_detection_thresholds_static.argtypes = [P, P, I64, I32, P, P]
         lib.linmin_detect.argtypes = [P, P, P, P, ctypes.c_float, I64, I32, P, P, P]
         lib.linmin_second_pass.argtypes = [P, P, P, I64, I32, I32, P, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_autofit.argtypes = [P, I32, I32, P, P, P]
@@ -424,6 +427,27 @@ def detection_thresholds(coeffs, present):
         _check(load().linmin_detection_thresholds(_dev_ptr(coeffs, "coeffs"), ctypes.c_void_p(present.data_ptr()), N, R,
                                                   _dev_ptr(thr, "thr"), _stream()))
     return thr
+
+
+def detection_thresholds_static(coeffs, present, out):
+    """linmin_detection_thresholds_static: eq. 8 thresholds without any device allocation by the library.
+
+    For callers whose GPU memory is all spoken for (an application-owned arena) or who cannot afford an
+    allocation's stall: the partial sums live in a fixed 384 KiB array inside liblinmin.so.  Nothing is allocated
+    here either: `present` must already be uint8 (or bool, viewed in place) and `out` is the caller's (R,) float32
+    tensor, returned filled.  R <= STATIC_MAX_R (64), else LinminError(ERR_STATIC_SCRATCH).  Calls on one device
+    share the array: keep them in stream order, and make the first one before any stream capture."""
+    torch = _torch()
+    N, R = int(coeffs.shape[0]), int(coeffs.shape[1])
+    if present.dtype == torch.bool:
+        present = present.view(torch.uint8)
+    _check_tensor(coeffs, "coeffs", (N, R), torch.float32, True)
+    _check_tensor(present, "present", (N, R), torch.uint8, True, coeffs.device)
+    _check_tensor(out, "out", (R,), torch.float32, True, coeffs.device)
+    with torch.cuda.device(coeffs.device):
+        _check(load().linmin_detection_thresholds_static(_dev_ptr(coeffs, "coeffs"), ctypes.c_void_p(present.data_ptr()),
+                                                         N, R, _dev_ptr(out, "out"), _stream()))
+    return out
 
 
 def detect(coeffs, coeff_sigma, resid, thresholds, rms_max):

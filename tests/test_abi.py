@@ -34,7 +34,7 @@ def test_exports_match_header(lib):
 def test_version_and_strerror(lib):
     from paper_1402_2518_b200 import linmin
     assert linmin.version() == 200
-    for code in [0, -1, -2, -3, -4, -5, -6, -7, 1]:
+    for code in [0, -1, -2, -3, -4, -5, -6, -7, -8, 1]:
         assert "unknown" not in linmin.strerror(code)
     assert "unknown" in linmin.strerror(12345)
 
