@@ -17,6 +17,19 @@ def test_eq8_hand_worked_golden():
     np.testing.assert_allclose(thr[0], expected, rtol=1e-14)
 
 
+def test_detect_hand_worked_golden():
+    """PAPER.md:241-246: each of the three conditions alone flips the entries the file says (derivation in the file);
+    a swapped comparison, a non-strict one, a shared threshold or a wrong broadcast of the RMS fails a row."""
+    rows = np.loadtxt(os.path.join(HERE, "golden", "detect_hand_worked.txt"))
+    par, data = rows[rows[:, 6] < 0][0], rows[rows[:, 6] >= 0]
+    thr, rms_max = par[:2], par[2]
+    mask, counts = D.detect(data[:, 0:2], data[:, 2:4], data[:, 4], thr, rms_max)
+    expected = data[:, 5:7] > 0.5
+    assert data.shape[0] == 11 and mask.shape == (11, 2)
+    assert np.array_equal(mask, expected), np.nonzero(mask != expected)
+    assert np.array_equal(counts, expected.sum(0)) and list(counts) == [6, 5]
+
+
 def test_eq8_against_a_vectorised_restatement_and_edge_cases():
     rng = np.random.default_rng(0)
     N, R = 500, 6
