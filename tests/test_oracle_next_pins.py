@@ -261,3 +261,33 @@ def test_weighted_rejects_indefinite_covariance():
     C = -np.eye(w.L, dtype=np.float32)
     with pytest.raises(ValueError):
         oracle.solve(w.A, w.Y, cov=C)
+
+
+@pytest.mark.parametrize("constraint,weighted", [("sto", False), ("pos", False), ("slo", False), ("sto", True), ("slo", True)])
+def test_tie_sigma_helper_of_the_parity_checks_agrees_with_the_oracle(constraint, weighted):
+    """tests/parity.py::sigma_reference_next is what the GPU's uncertainties are held to on tie pixels (R10).  It is
+    written from R3 / R17 with numpy's inverse in coefficient space; the oracle goes through a QR in data space.
+    Two routes, one quantity: they must agree on the oracle's own support, for every option."""
+    import sys, os
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    from parity import sigma_reference_next
+    w = make_workload("tiny", N=60)
+    rng = np.random.default_rng(5)
+    Y = (w.Y * rng.uniform(0.6, 1.1, size=(w.N, 1))).astype(np.float32)          # sums below and at one
+    cov = None
+    if weighted:
+        s = rng.uniform(0.002, 0.01, w.L)
+        idx = np.arange(w.L)
+        cov = ((0.5 ** np.abs(idx[:, None] - idx[None, :])) * np.outer(s, s)).astype(np.float32)
+    ora = oracle.solve(w.A, Y, None if weighted else w.sigma, constraint=constraint, cov=cov)
+    Ci = np.linalg.inv(cov.astype(np.float64)) if weighted else None
+    A64 = w.A.astype(np.float64)
+    seen = set()
+    for p in range(w.N):
+        a = ora.coeffs[p]
+        eq = constraint == "sto" or (constraint == "slo" and a.sum() >= 1 - 1e-9)
+        seen.add(eq)
+        ref = sigma_reference_next(A64, np.nonzero(a > 0)[0], eq, Ci, None if weighted else w.sigma[p])
+        np.testing.assert_allclose(ora.coeff_sigma[p], ref, rtol=1e-6, atol=1e-12)
+    if constraint == "slo":
+        assert seen == {True, False}
