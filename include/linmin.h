@@ -26,6 +26,12 @@
  *                                    stride s >= L   -> per pixel, sigma[p*s + l]
  *   coeffs_out[p*R + r], coeff_sigma_out[p*R + r], resid_out[p]
  *
+ * Alignment: float32 alignment (4 bytes) is all that is required of any array.  The fast kernels use 16-byte
+ * accesses where the arrays allow it: Y (and per-pixel sigma) 16-byte aligned with ldY (the stride) a multiple of
+ * 4, coeffs_out / coeff_sigma_out 16-byte aligned.  Arrays that are not take scalar paths -- at R = 32 a coeffs_out
+ * that is not 16-byte aligned sends IPLS through the any-size kernel, several times slower; results are the same
+ * minimiser either way (every pixel is finished exactly).
+ *
  * Ownership: every pointer is owned by the caller; the library never frees or reallocates caller
  * memory.  Outputs must not alias inputs or each other.  `coeff_sigma_out`, `resid_out`, `sigma`
  * and `opts` may be NULL (output skipped / defaults).  Internal workspace (O(R^2 + L R) bytes) is
@@ -107,6 +113,8 @@ extern "C" {
 #define LINMIN_INFO_FINISH_FALLBACK 0x10 /* finish hit its pivot/support cap: result feasible, near-optimal, not certified */
 #define LINMIN_INFO_BAD_SIGMA 0x20      /* sigma <= 0 or non-finite: coeff_sigma of the pixel is NaN */
 #define LINMIN_INFO_LIBRARY_NONFINITE 0x40 /* linmin_unmix only: A holds NaN/Inf, every output of the call is NaN */
+#define LINMIN_INFO_COVARIANCE 0x80     /* linmin_unmix only: opts->cov is not finite / not positive definite, every
+                                           output of the call is NaN */
 #define LINMIN_INFO_ITERATIONS(w) (((w) >> 8) & 0xff)  /* IPLS Newton iterations */
 #define LINMIN_INFO_PIVOTS(w) (((w) >> 16) & 0xff)     /* finish support changes */
 #define LINMIN_INFO_SUPPORT(w) (((w) >> 24) & 0xff)    /* number of non-zero coefficients */
@@ -154,9 +162,13 @@ int linmin_unmix_lib(const linmin_library *lib, const float *Y, const float *sig
                      float *resid_out);
 
 /* One-shot form: precompute + solve + release, all enqueued on opts->stream; returns without waiting.
- * Device pointers.  Since nothing is read back, a non-finite library is reported through the OUTPUTS:
- * all of them NaN, every info word = LINMIN_INFO_LIBRARY_NONFINITE (linmin_library_create reports
- * it as a status instead). */
+ * Device pointers.  Since nothing is read back, a non-finite library and a covariance that is not positive
+ * definite are reported through the OUTPUTS: all of them NaN, every info word = LINMIN_INFO_LIBRARY_NONFINITE
+ * and / or LINMIN_INFO_COVARIANCE (linmin_library_create reports them as a status instead:
+ * LINMIN_ERR_LIBRARY_NONFINITE, LINMIN_ERR_COVARIANCE).
+ * Cost: every call repeats the once-per-library precompute, part of which runs on ONE thread block (start-point data,
+ * O(R^3); with a covariance its Cholesky factor and inverse, O(L^3): a few milliseconds at L = 512).  For more
+ * than one cube against the same library use linmin_library_create + linmin_unmix_lib. */
 int linmin_unmix(const float *A, const float *Y, const float *sigma, int64_t N, int32_t L, int32_t R,
                  const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out, float *resid_out);
 
@@ -173,8 +185,11 @@ int linmin_library_last_launches(const linmin_library *lib);
 /* Per-kernel timing for reports (bench.py's roofline): when enabled, linmin_unmix_lib brackets each
  * of its kernels with CUDA events on the call's stream.  linmin_library_last_timing blocks until the
  * last call's events have completed and returns the device time of the projection+IPLS kernel and of
- * the finish/uncertainty/residual kernel in milliseconds.  Returns LINMIN_ERR_INVALID_ARGUMENT when
- * timing is disabled or no call was made.  Not thread-safe per handle. */
+ * the finish/uncertainty/residual kernel in milliseconds.  The two always add up to the whole call; with
+ * sum-lower-than-one at R = 32 (two passes, see LINMIN_CONSTRAINT_SUM_LOWER_THAN_ONE) ipls_ms holds the whitening,
+ * the whole positivity-only pass and the IPLS kernels of the sum-to-one pass, finish_ms the sum-to-one finish and
+ * the per-pixel selection.  Returns LINMIN_ERR_INVALID_ARGUMENT when timing is disabled or no call was made.
+ * Not thread-safe per handle. */
 int linmin_library_enable_timing(linmin_library *lib, int enable);
 int linmin_library_last_timing(const linmin_library *lib, float *ipls_ms, float *finish_ms);
 

@@ -202,13 +202,14 @@ void note_use(const linmin_library *lib, cudaStream_t stream) {
 
 // prewhitened: Y is already Y W' (the caller did the renormalisation of this handle's covariance)
 int solve_core(const linmin_library *lib, const float *Y, const float *sigma, int64_t N,
-               const Resolved &o, float *coeffs, float *csig, float *resid, bool prewhitened) {
+               const Resolved &o, float *coeffs, float *csig, float *resid, bool prewhitened,
+               bool record_start = true) {
     const int L = lib->L, R = lib->Ri;      // R: the endmembers the kernels see (slack included)
     const bool cons = lib->constraint != LINMIN_CONSTRAINT_POSITIVITY_ONLY;
     LibView lv = view_of(lib);
     struct FreeV { void *p; cudaStream_t s; ~FreeV() { if (p) cudaFreeAsync(p, s); } };
     int launches = 0;
-    if (lib->timing) CK(cudaEventRecord(lib->ev[0], o.stream));
+    if (lib->timing && record_start) CK(cudaEventRecord(lib->ev[0], o.stream));
     int64_t ldY = o.ldY, sstride = o.sstride;
     // ---- renormalised problem (eq. 6): Y' = Y W' into a workspace, then the unweighted path on
     //      (A', Y') with unit noise
@@ -253,7 +254,10 @@ int solve_core(const linmin_library *lib, const float *Y, const float *sigma, in
     CK(cudaMemsetAsync(ws, 0, std::min<size_t>(9, ws_words) * sizeof(unsigned int), o.stream));
     unsigned int *counters = ws, *overflow = ws + 8, *repair = ws + 8 + ((size_t)N + 1);
     if (use_f8) CK(cudaMemsetAsync(repair, 0, sizeof(unsigned int), o.stream));
-    if (R == 32 && start_r32_warps(L) > 0) {
+    // K1 hands its iterate over with 16-byte stores: a coeffs_out that is only 4-byte aligned (a sub-view of a larger
+    // buffer) takes the any-size IPLS kernel instead (scalar stores; same minimiser, the finish is exact either way)
+    const bool coeffs16 = (reinterpret_cast<uintptr_t>(coeffs) & 15) == 0;
+    if (R == 32 && start_r32_warps(L) > 0 && coeffs16) {
         // K0 (projection + start point, one record per pixel) and K1 (the iteration), in chunks of 2^21 pixels
         // so that the record workspace stays at 0.8 GB whatever N is
         const int64_t chunk = (int64_t)1 << 21;
@@ -356,6 +360,9 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     Resolved oc = o;
     float *Yw = nullptr;
     int extra = 0;
+    // timing report: the call starts here and ends after the selection; the first interval then holds the whitening,
+    // the whole pos pass and the IPLS kernels of the sto pass, the second the sto finish and the selection
+    if (lib->timing) CK(cudaEventRecord(lib->ev[0], o.stream));
     if (lib->weighting != LINMIN_WEIGHTING_NONE) {
         CK(staging_alloc((void **)&Yw, (size_t)N * L * sizeof(float), o.stream));
         CK(launch_whiten_spectra(Y, o.ldY, N, L, lib->W, lib->weighting == LINMIN_WEIGHTING_SHARED_DIAGONAL, Yw,
@@ -378,11 +385,12 @@ int launch_solve(const linmin_library *lib, const float *Y, const float *sigma, 
     op.info = ip;
     int rc = solve_core(lib->pos_twin, Y, sigma, N, op, cp, sp, rp, true);
     if (rc != LINMIN_OK) return rc;
-    rc = solve_core(lib, Y, sigma, N, oc, coeffs, csig, resid, true);
+    rc = solve_core(lib, Y, sigma, N, oc, coeffs, csig, resid, true, false);
     if (rc != LINMIN_OK) return rc;
     const int grid = (int)std::min<int64_t>((N + 7) / 8, (int64_t)lib->sm_count * 16);
     slo_select_kernel<<<grid, 256, 0, o.stream>>>(N, R, cp, sp, rp, ip, coeffs, csig, resid, o.info);
     CK(cudaGetLastError());
+    if (lib->timing) CK(cudaEventRecord(lib->ev[2], o.stream));
     lib->last_launches.store(lib->last_launches.load() + lib->pos_twin->last_launches.load() + extra + 1);
     return LINMIN_OK;
 }

@@ -134,11 +134,14 @@ start_data_kernel(const float *__restrict__ Gc, int R, double *__restrict__ W, f
     if (tid == 0) scal[2] = (float)tsh;
 }
 
-// One-shot calls do not wait for the library check: when the library turned out non-finite, every output of the
-// call is overwritten with NaN and every info word with LINMIN_INFO_LIBRARY_NONFINITE (include/linmin.h).
+// One-shot calls do not wait for the library check: when the library turned out non-finite (flag bit 0) or the noise
+// covariance not positive definite (bit 1), every output of the call is overwritten with NaN and every info word with
+// LINMIN_INFO_LIBRARY_NONFINITE and / or LINMIN_INFO_COVARIANCE (include/linmin.h).
 __global__ void poison_outputs_kernel(const int *__restrict__ flags, int64_t N, int R, float *__restrict__ coeffs,
                                       float *__restrict__ csig, float *__restrict__ resid, int32_t *__restrict__ info) {
-    if (!flags[0]) return;
+    const int f = flags[0];
+    if (!f) return;
+    const int32_t word = ((f & 1) ? LINMIN_INFO_LIBRARY_NONFINITE : 0) | ((f & 2) ? LINMIN_INFO_COVARIANCE : 0);
     const float qnan = __int_as_float(0x7fc00000);
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < N * R; e += stride) {
@@ -147,7 +150,7 @@ __global__ void poison_outputs_kernel(const int *__restrict__ flags, int64_t N, 
     }
     for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < N; p += stride) {
         if (resid) resid[p] = qnan;
-        if (info) info[p] = LINMIN_INFO_LIBRARY_NONFINITE;
+        if (info) info[p] = word;
     }
 }
 

@@ -48,13 +48,35 @@ whitening_matrix_kernel(const float *__restrict__ cov, int kind, int L, double *
         }
         __syncthreads();
     }
-    // W = Rc^-1: one thread per column (forward substitution of a unit vector)
-    for (int c = tid; c < L; c += nt) {
-        for (int i = 0; i < c; ++i) Wd[(size_t)i * L + c] = 0.0;
-        for (int i = c; i < L; ++i) {
-            double v = (i == c) ? 1.0 : 0.0;
-            for (int k = c; k < i; ++k) v -= Cd[(size_t)i * L + k] * Wd[(size_t)k * L + c];
-            Wd[(size_t)i * L + c] = v / Cd[(size_t)i * L + i];
+    // W = Rc^-1 by forward substitution of the unit vectors: one WARP per column, the column in registers (entry k
+    // on lane k mod 32), the dot product of row i split over the lanes (coalesced reads of Rc's row) and summed by
+    // shuffles -- L steps of L / 32 products per column instead of one thread's chain of L^2 / 2 dependent loads
+    {
+        const int lane = tid & 31, wid = tid >> 5, nw = nt >> 5;
+        constexpr int M = LINMIN_MAX_L / 32;
+        for (int c = wid; c < L; c += nw) {
+            double x[M];
+#pragma unroll
+            for (int m = 0; m < M; ++m) x[m] = 0.0;
+            for (int i = c; i < L; ++i) {
+                const double *row = Cd + (size_t)i * L;
+                double v = 0.0;
+#pragma unroll
+                for (int m = 0; m < M; ++m) {
+                    const int k = lane + 32 * m;
+                    if (k < i) v += row[k] * x[m];          // (entries above the column's first row are still zero)
+                }
+                v = warp_sum(v);
+                const double xi = (((i == c) ? 1.0 : 0.0) - v) / row[i];
+#pragma unroll
+                for (int m = 0; m < M; ++m)
+                    if (lane + 32 * m == i) x[m] = xi;
+            }
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                const int k = lane + 32 * m;
+                if (k < L) Wd[(size_t)k * L + c] = x[m];
+            }
         }
     }
     __syncthreads();

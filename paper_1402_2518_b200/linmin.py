@@ -35,6 +35,7 @@ INFO_CHOL_REGULARISED = 0x08
 INFO_FINISH_FALLBACK = 0x10
 INFO_BAD_SIGMA = 0x20
 INFO_LIBRARY_NONFINITE = 0x40
+INFO_COVARIANCE = 0x80
 
 EXPORTS = ["linmin_version", "linmin_strerror", "linmin_library_create", "linmin_library_destroy",
            "linmin_library_last_launches", "linmin_library_enable_timing", "linmin_library_last_timing",

@@ -112,6 +112,45 @@ def test_library_handle_strides_shared_sigma_and_host_path(lm):
     lib.destroy()
 
 
+@pytest.mark.parametrize("constraint", [0, 1, 2])
+def test_arrays_need_only_float_alignment(lm, constraint):
+    """include/linmin.h, "Alignment": every array may sit on any 4-byte boundary.  R = 32 is the size whose IPLS kernel
+    stores 16 bytes at a time; outputs (and Y, sigma) that are sub-views one float into a larger buffer must give the
+    oracle's result, not a misaligned-address fault."""
+    import oracle
+    from paper_1402_2518_b200.synth import make_workload
+    from parity import check_parity, check_parity_next
+    w = make_workload("omega", N=1003)
+    dev = torch.device("cuda:0")
+    assert w.R == 32
+
+    def off1(shape, dtype=torch.float32, src=None):
+        n = int(np.prod(shape))
+        buf = torch.zeros(n + 1, dtype=dtype, device=dev)
+        v = buf[1:].view(*shape)
+        if src is not None:
+            v.copy_(torch.from_numpy(src).to(dev))
+        assert v.data_ptr() % 16 == 4 and v.is_contiguous()
+        return v
+
+    Y, S = off1((w.N, w.L), src=w.Y), off1((w.N, w.L), src=w.sigma)
+    out = dict(coeffs=off1((w.N, w.R)), coeff_sigma=off1((w.N, w.R)), resid=off1((w.N,)), info=off1((w.N,), torch.int32))
+    c, s, r, info, st = lm.unmix(torch.from_numpy(w.A).to(dev), Y, S, out=out, constraint=constraint)
+    torch.cuda.synchronize()
+    assert c.data_ptr() == out["coeffs"].data_ptr()
+    g = dict(coeffs=c.cpu().numpy(), coeff_sigma=s.cpu().numpy(), resid=r.cpu().numpy())
+    if constraint == 0:
+        check_parity(w.A, w.Y, w.sigma, g, oracle.solve(w.A, w.Y, w.sigma), label="misaligned")
+    else:
+        name = {1: "slo", 2: "pos"}[constraint]
+        check_parity_next(w.A, w.Y, g, oracle.solve(w.A, w.Y, w.sigma, constraint=name), constraint=name,
+                          label="misaligned/" + name, sigma=w.sigma)
+    # same minimiser as with aligned arrays (another IPLS kernel hands over, the finish is exact)
+    ca = lm.unmix(torch.from_numpy(w.A).to(dev), torch.from_numpy(w.Y).to(dev), torch.from_numpy(w.sigma).to(dev),
+                  constraint=constraint)[0]
+    assert float((ca - c).abs().max()) < 1e-5
+
+
 def test_empty_single_and_determinism(lm):
     from paper_1402_2518_b200.synth import make_workload
     w = make_workload("tiny", N=9)
@@ -181,12 +220,31 @@ def test_degenerate_inputs(lm):
     gb = run_gpu(lm, Ab, Y, np.full((20, L), 0.01, np.float32))
     assert np.isnan(gb["coeffs"]).all() and np.isnan(gb["coeff_sigma"]).all() and np.isnan(gb["resid"]).all()
     assert (gb["info"] == lm.INFO_LIBRARY_NONFINITE).all()
+    # same contract for a covariance that is not positive definite on the one-shot path: its own info bit
+    Cbad = -np.eye(L, dtype=np.float32)
+    t = lambda x: torch.from_numpy(x).to("cuda:0")
+    with pytest.raises(lm.LinminError) as e:
+        lm.library_create(t(A), cov=t(Cbad))
+    assert e.value.code == lm.ERR_COVARIANCE
+    for lib_arr, word in ((A, lm.INFO_COVARIANCE), (Ab, lm.INFO_COVARIANCE | lm.INFO_LIBRARY_NONFINITE)):
+        c, s, r, info, _ = lm.unmix(t(lib_arr), t(Y), None, cov=t(Cbad))
+        torch.cuda.synchronize()
+        assert torch.isnan(c).all() and torch.isnan(s).all() and torch.isnan(r).all()
+        assert (info.cpu().numpy() == word).all()
+    sdiag = np.full(L, 0.01, np.float32); sdiag[2] = 0.0            # a zero noise std: diagonal covariance refused too
+    c, s, r, info, _ = lm.unmix(t(A), t(Y), None, cov=t(sdiag))
+    torch.cuda.synchronize()
+    assert torch.isnan(c).all() and (info.cpu().numpy() == lm.INFO_COVARIANCE).all()
     # a zero endmember (what a sum-lower-than-one slack column looks like): results stay on the simplex
     Az = np.concatenate([A, np.zeros((L, 1), np.float32)], axis=1)
     gz = run_gpu(lm, Az, Y, None)
     oz = oracle.solve(Az, Y)
     assert np.abs(gz["coeffs"].sum(1) - 1).max() <= 1e-5 and gz["coeffs"].min() >= 0
     np.testing.assert_allclose(gz["resid"], oz.resid, rtol=1e-5)
+    # ... element by element: coefficients, uncertainties, residual within the parity tolerances
+    from parity import check_parity
+    check_parity(Az, Y, np.ones(L, np.float32), gz, oz, label="zero endmember")
+    assert (oz.coeffs[:, -1] > 0).any() and (oz.coeffs[:, -1] == 0).any()     # the slack is used by some pixels only
 
 
 def test_boundary_is_asynchronous_graph_capturable_and_stream_safe(lm):
