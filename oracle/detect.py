@@ -40,15 +40,21 @@ def additional_spectra(L: int, n_extra: int, wavelength=None) -> np.ndarray:
     return np.stack(cols, axis=1)
 
 
-def thresholds(coeffs: np.ndarray, present: np.ndarray) -> np.ndarray:
-    """eq. 8, one value per endmember.  coeffs (N, R) estimated, present (N, R) bool: i belongs to the true mixture."""
+def thresholds(coeffs: np.ndarray, present: np.ndarray, whole_class: bool = False) -> np.ndarray:
+    """eq. 8, one value per endmember.  coeffs (N, R) estimated, present (N, R) bool: i belongs to the true mixture.
+    whole_class False (reading R19): A+ / A- are the DETECTIONS (estimate > 0) on present / absent pixels, the green
+    and red points of Fig. 4 ("in the case of positive / false detection").  whole_class True (the alternative reading
+    of PAPER.md:131, "~30 ... with non-null mixing coefficient (noted A^positive) and ~970 with null mixing coefficient
+    (A^false)"): every pixel of each class enters, estimates of exactly 0 included -- what an interior-point iterate
+    that never returns an exact 0 would feed eq. 8."""
     coeffs = np.asarray(coeffs, dtype=np.float64)
     present = np.asarray(present, dtype=bool)
     R = coeffs.shape[1]
     out = np.zeros(R)
     for i in range(R):
-        pos = coeffs[present[:, i] & (coeffs[:, i] > 0), i]
-        neg = coeffs[~present[:, i] & (coeffs[:, i] > 0), i]
+        counted = np.ones(coeffs.shape[0], dtype=bool) if whole_class else (coeffs[:, i] > 0)
+        pos = coeffs[present[:, i] & counted, i]
+        neg = coeffs[~present[:, i] & counted, i]
         mp, sp = (pos.mean(), pos.std()) if len(pos) else (0.0, 0.0)
         mf, sf = (neg.mean(), neg.std()) if len(neg) else (0.0, 0.0)
         out[i] = 0.5 * (mp - 2.0 * sp + mf + 6.0 * sf)

@@ -17,6 +17,20 @@ def test_eq8_hand_worked_golden():
     np.testing.assert_allclose(thr[0], expected, rtol=1e-14)
 
 
+def test_eq8_whole_class_hand_worked_golden():
+    """The alternative reading of PAPER.md:131 (every pixel of a class, exact zeros included): its own hand-worked
+    value on the same eight pixels, and it differs from reading R19's."""
+    rows = np.loadtxt(os.path.join(HERE, "golden", "eq8_whole_class_hand_worked.txt"))
+    data, expected = rows[rows[:, 1] >= 0], rows[rows[:, 1] < 0][0, 0]
+    thr = D.thresholds(data[:, :1], data[:, 1:2] > 0.5, whole_class=True)
+    np.testing.assert_allclose(thr[0], expected, rtol=1e-14)
+    assert abs(D.thresholds(data[:, :1], data[:, 1:2] > 0.5)[0] - expected) > 0.1
+    # an estimator that never returns an exact zero (the paper's interior-point iterate): both readings coincide
+    rng = np.random.default_rng(3)
+    c = rng.uniform(1e-6, 0.5, (200, 3)); present = rng.uniform(size=(200, 3)) < 0.2
+    np.testing.assert_allclose(D.thresholds(c, present, whole_class=True), D.thresholds(c, present), rtol=1e-14)
+
+
 def test_detect_hand_worked_golden():
     """PAPER.md:241-246: each of the three conditions alone flips the entries the file says (derivation in the file);
     a swapped comparison, a non-strict one, a shared threshold or a wrong broadcast of the RMS fails a row."""
