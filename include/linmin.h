@@ -218,7 +218,16 @@ int linmin_additional_spectra(const float *wavelength, int32_t L, int32_t n_extr
 int linmin_detection_thresholds(const float *coeffs, const unsigned char *present, int64_t N, int32_t R,
                                 float *thresholds_out, void *stream);
 
-/* The same thresholds for callers that cannot let the library allocate device memory: an application that gave the
+/* The same with the class definition as an argument.  whole_class = 0: as above (reading R19: A+ / A- are the
+ * detections, estimate > 0 -- the green / red points of the paper's Fig. 4).  whole_class = 1: every pixel of each
+ * class enters the mean and the std, estimates of exactly 0 included -- PAPER.md:131 defines the classes by the TRUE
+ * coefficient ("~30 ... non-null ... A^positive", "~970 ... null ... A^false"), and the paper's interior-point
+ * iterate never returns an exact 0, so this is what its eq. 8 ran over; here the exact finish returns exact zeros
+ * for most absent endmembers and the two readings differ (R19 has the measured size). */
+int linmin_detection_thresholds_ex(const float *coeffs, const unsigned char *present, int64_t N, int32_t R,
+                                   int32_t whole_class, float *thresholds_out, void *stream);
+
+/* The thresholds of linmin_detection_thresholds (whole_class = 0) for callers that cannot let the library allocate device memory: an application that gave the
  * whole GPU to its own arena at start-up (an allocation made here would fail or take memory it has planned for),
  * or a latency-bound loop that cannot afford the device-wide synchronisation and unbounded duration an allocation
  * may cost.  linmin_detection_thresholds draws its per-block partial sums from the library's staging pool; this
@@ -248,7 +257,8 @@ int linmin_detect(const float *coeffs, const float *coeff_sigma, const float *re
 
 /* Second pass "with the detected spectrum only": linmin_unmix against the columns of A whose byte in
  * keep (R bytes, device) is non-zero; coefficients and uncertainties of the other endmembers are 0.  SYNCHRONISES
- * opts->stream once (the size of the sub-library decides the allocations). */
+ * opts->stream TWICE: once to read `keep` (the size of the sub-library decides the allocations) and once after
+ * uploading the column list (a host array that does not outlive the call).  Not capturable into a CUDA graph. */
 int linmin_second_pass(const float *A, const float *Y, const float *sigma, int64_t N, int32_t L, int32_t R,
                        const unsigned char *keep, const linmin_opts *opts, float *coeffs_out, float *coeff_sigma_out,
                        float *resid_out);

@@ -40,18 +40,18 @@ __global__ void additional_spectra_kernel(const float *__restrict__ wavelength, 
     }
 }
 
-// ---- eq. 8.  Stage 1: block b accumulates, for each endmember, (count, sum, sum of squares) of the detections (> 0)
-// on present / absent pixels in fp64; a thread stays on ONE column (blockDim.x is a multiple of R), so the loads are
+// ---- eq. 8.  Stage 1: block b accumulates, for each endmember, (count, sum, sum of squares) of the detections (> 0;
+// with whole_class: of every estimate) on present / absent pixels in fp64; a thread stays on ONE column (blockDim.x is a multiple of R), so the loads are
 // coalesced and the per-thread sums need no exchange until the end.  part: [gridDim.x][R][6].
 __global__ void threshold_partial_kernel(const float *__restrict__ coeffs, const unsigned char *__restrict__ present,
-                                         int64_t N, int R, double *__restrict__ part) {
+                                         int64_t N, int R, int whole_class, double *__restrict__ part) {
     extern __shared__ double sh[];          // [blockDim.x][6]
     const int64_t total = N * R;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     double acc[6] = {0, 0, 0, 0, 0, 0};
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += stride) {
         const float v = coeffs[e];
-        if (v > 0.0f) {
+        if (whole_class || v > 0.0f) {          // whole_class: every pixel of the class, exact zeros included
             const int o = present[e] ? 0 : 3;
             acc[o] += 1.0; acc[o + 1] += (double)v; acc[o + 2] += (double)v * (double)v;
         }

@@ -725,7 +725,13 @@ int linmin_additional_spectra(const float *wavelength, int32_t L, int32_t n_extr
 
 int linmin_detection_thresholds(const float *coeffs, const unsigned char *present, int64_t N, int32_t R,
                                 float *thresholds_out, void *stream) {
+    return linmin_detection_thresholds_ex(coeffs, present, N, R, 0, thresholds_out, stream);
+}
+
+int linmin_detection_thresholds_ex(const float *coeffs, const unsigned char *present, int64_t N, int32_t R,
+                                   int32_t whole_class, float *thresholds_out, void *stream) {
     if (!coeffs || !present || !thresholds_out || N < 0 || R < 1) return LINMIN_ERR_INVALID_ARGUMENT;
+    if (whole_class != 0 && whole_class != 1) return LINMIN_ERR_INVALID_ARGUMENT;
     if (R > LINMIN_MAX_R) return LINMIN_ERR_UNSUPPORTED_SIZE;
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, sms = 0;
@@ -735,7 +741,7 @@ int linmin_detection_thresholds(const float *coeffs, const unsigned char *presen
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N * R + block - 1) / block, (int64_t)sms * 8));
     double *part = nullptr;
     CK(staging_alloc((void **)&part, (size_t)grid * R * 6 * sizeof(double), st));
-    threshold_partial_kernel<<<grid, block, (size_t)block * 6 * sizeof(double), st>>>(coeffs, present, N, R, part);
+    threshold_partial_kernel<<<grid, block, (size_t)block * 6 * sizeof(double), st>>>(coeffs, present, N, R, whole_class, part);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) {
         threshold_final_kernel<<<(R + 63) / 64, 64, 0, st>>>(part, grid, R, thresholds_out);

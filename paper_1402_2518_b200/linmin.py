@@ -41,7 +41,7 @@ EXPORTS = ["linmin_version", "linmin_strerror", "linmin_library_create", "linmin
            "linmin_library_last_launches", "linmin_library_enable_timing", "linmin_library_last_timing",
            "linmin_trim_memory",
            "linmin_unmix_lib", "linmin_unmix", "linmin_unmix_host",
-           "linmin_additional_spectra", "linmin_detection_thresholds", "linmin_detection_thresholds_static", "linmin_detect", "linmin_second_pass",
+           "linmin_additional_spectra", "linmin_detection_thresholds", "linmin_detection_thresholds_ex", "linmin_detection_thresholds_static", "linmin_detect", "linmin_second_pass",
            "linmin_autofit"]
 
 
@@ -86,6 +86,7 @@ def load() -> ctypes.CDLL:
         lib.linmin_unmix_host.argtypes = [P, P, P, I64, I32, I32, ctypes.POINTER(LinminOpts), P, P, P]
         lib.linmin_additional_spectra.argtypes = [P, I32, I32, P, I32, I32, P]
         lib.linmin_detection_thresholds.argtypes = [P, P, I64, I32, P, P]
+        lib.linmin_detection_thresholds_ex.argtypes = [P, P, I64, I32, I32, P, P]
         lib.linmin_detection_thresholds_static.argtypes = [P, P, I64, I32, P, P]
         lib.linmin_detect.argtypes = [P, P, P, P, ctypes.c_float, I64, I32, P, P, P]
         lib.linmin_second_pass.argtypes = [P, P, P, I64, I32, I32, P, ctypes.POINTER(LinminOpts), P, P, P]
@@ -416,8 +417,9 @@ def build_library(A_ref, n_extra, wavelength=None):
     return additional_spectra(L, n_extra, A_ref.device, wavelength, out, R0)
 
 
-def detection_thresholds(coeffs, present):
-    """linmin_detection_thresholds (eq. 8): coeffs (N, R) float32, present (N, R) uint8 / bool -> (R,) float32."""
+def detection_thresholds(coeffs, present, whole_class=False):
+    """linmin_detection_thresholds[_ex] (eq. 8): coeffs (N, R) float32, present (N, R) uint8 / bool -> (R,) float32.
+    whole_class: every pixel of a class enters, exact zeros included, instead of the detections only."""
     torch = _torch()
     N, R = int(coeffs.shape[0]), int(coeffs.shape[1])
     present = present.to(torch.uint8)
@@ -425,8 +427,8 @@ def detection_thresholds(coeffs, present):
     _check_tensor(present, "present", (N, R), torch.uint8, True, coeffs.device)
     thr = torch.empty((R,), dtype=torch.float32, device=coeffs.device)
     with torch.cuda.device(coeffs.device):
-        _check(load().linmin_detection_thresholds(_dev_ptr(coeffs, "coeffs"), ctypes.c_void_p(present.data_ptr()), N, R,
-                                                  _dev_ptr(thr, "thr"), _stream()))
+        _check(load().linmin_detection_thresholds_ex(_dev_ptr(coeffs, "coeffs"), ctypes.c_void_p(present.data_ptr()), N, R,
+                                                     int(bool(whole_class)), _dev_ptr(thr, "thr"), _stream()))
     return thr
 
 

@@ -192,6 +192,16 @@ def test_library_builder_detection_layer_and_second_pass(lm):
     np.testing.assert_allclose(thr.cpu().numpy(), thr_ref, rtol=2e-6, atol=1e-9)
     thr2 = lm.detection_thresholds(c, present)
     assert torch.equal(thr, thr2)                                   # fixed summation order
+    # the whole-class reading of PAPER.md:131 (exact zeros enter the class statistics), and how far it is from R19
+    thr_wc = lm.detection_thresholds(c, present, whole_class=True)
+    np.testing.assert_allclose(thr_wc.cpu().numpy(), D.thresholds(cn, w.a0 > 0, whole_class=True), rtol=2e-6, atol=1e-9)
+    print("eq. 8 on the labelled omega set: R19 mean threshold %.4f, whole-class %.4f, median ratio %.2f" % (
+        float(thr.mean()), float(thr_wc.mean()), float((thr_wc / thr).median())))
+    raw = lm.load().linmin_detection_thresholds      # the plain C entry point is the R19 reading
+    thr3 = torch.empty_like(thr)
+    assert raw(c.data_ptr(), present.to(torch.uint8).data_ptr(), w.N, w.R, thr3.data_ptr(), None) == 0
+    torch.cuda.synchronize()
+    assert torch.equal(thr3, thr)
     # detection mask: bit-exact against the definition evaluated on the same float32 arrays
     rms_max = 0.0065
     mask, counts = lm.detect(c, s, r, thr, rms_max)
