@@ -6,7 +6,8 @@
 One "step" = one pass of the whole hot path (projection, IPLS, exact finish, uncertainty
 propagation, residual, output store) over the workload.  At N = 1 the workload is BASELINE.json
 configs[4] ("throughput": L = 128, R = 32, N = 16,777,216 = 128 OMEGA-like cubes, per-pixel sigma),
-synthetic and seeded (paper_1402_2518_b200/synth.py).  With --gpus N > 1 (launched by torchrun) every
+synthetic and seeded (paper_1402_2518_b200/synth.py).  With --gpus N > 1 (under torchrun, or plain: bench.py then
+starts its own N ranks through torch.distributed.run on 127.0.0.1 and refuses when fewer devices are visible) every
 rank owns its own 128 cubes ("weak" scaling; pixels are independent, no collective on the data path).
 `value` = spectra/s with inputs resident in HBM; `e2e` = the same through linmin_unmix_host with
 pinned HOST buffers (H2D and D2H inside the timed region).  `--impl reference` times the CPU fp64
@@ -29,7 +30,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_1402_2518_b200.shard import cube_block, max_over_ranks  # noqa: E402
+from paper_1402_2518_b200.shard import cube_block, launch_plan, max_over_ranks  # noqa: E402
 from paper_1402_2518_b200.synth import CONFIGS, make_cube, make_library  # noqa: E402
 
 METRIC = "unmixed spectra/sec"
@@ -240,6 +241,25 @@ def main():
                     help="skip the extra report keys (other configs, NEXT-row options); the headline is unaffected")
     args = ap.parse_args()
 
+    if args.impl == "ours":
+        # `python bench.py --gpus N` without torchrun starts its own N ranks (one per GPU, this node)
+        import socket
+        visible = 0
+        if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+            import torch
+            visible = torch.cuda.device_count()
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        try:
+            kind, cmd = launch_plan(args.gpus, os.environ, visible, [os.path.abspath(__file__)] + sys.argv[1:],
+                                    sys.executable, port)
+        except ValueError as e:
+            raise SystemExit(f"bench.py: {e}")
+        if kind == "spawn":
+            sys.stdout.flush()
+            os.execv(sys.executable, cmd)
+
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -338,20 +358,30 @@ def main():
     info = out["info"].cpu().numpy()
     it, piv, k = (info >> 8) & 0xff, (info >> 16) & 0xff, (info >> 24) & 0xff
     f_ipls, f_fin = flops_model(L, R, it, piv, k)
+    # per-pixel distributions behind the means (rank 0's pixels): index = value, entry = pixel count
+    histograms = {
+        "iterations": np.bincount(it).tolist(), "pivots": np.bincount(piv).tolist(), "support": np.bincount(k).tolist(),
+        "frac_support_above_16": float((k > 16).mean()),       # the pixels finish_sweep hands to finish_fast
+        "frac_with_support_change": float((piv > 0).mean()),   # the pixels of finish_sweep's second (repair) pass
+        "pixels": int(N),
+    }
     ipls_avg = float(np.mean(ipls_ms)); fin_avg = float(np.mean(fin_ms))
     achieved = f_ipls / (ipls_avg * 1e-3) / 1e12
     traffic = None
+    whole_dram = None
     tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
     if os.path.exists(tpath):
         try:
             tj = json.load(open(tpath))
             traffic = tj.get("ipls_kernel_dram_bytes_per_pixel", None)
+            keys = [kk for kk in tj if kk.endswith("_dram_bytes_per_pixel")]
+            whole_dram = float(sum(tj[kk] for kk in keys)) if keys else None     # every kernel of the step (stored ncu figures)
             if traffic is not None:      # K0 and K1 are timed together: both kernels' bytes
                 traffic = (traffic + tj.get("start_r32_kernel_dram_bytes_per_pixel", 0.0)) * N
         except (OSError, ValueError):
             traffic = None
     try:
-        from paper_1402_2518_b200.fp32_probe import probe_fp32_peak
+        from bench_probe.fp32_probe import probe_fp32_peak
         ffma_tf, ffma2_tf = probe_fp32_peak()
     except Exception:  # report helper only: never fail the bench line on it
         ffma_tf, ffma2_tf = None, None
@@ -374,6 +404,7 @@ def main():
         "whole_step": {"achieved": (f_ipls + f_fin) / (ms_step * 1e-3) / 1e12,
                        "frac": (f_ipls + f_fin) / (ms_step * 1e-3) / 1e12 / FP32_PEAK_TFLOPS},
         "hbm": {"algorithmic_bytes_per_pixel": 4 * L * 2 + 4 * (2 * R + 1) + 4,
+                "dram_bytes_per_pixel_whole_step_stored": whole_dram,
                 "achieved_GBps": (4 * L * 2 + 4 * (2 * R + 1) + 4) * N / (ms_step * 1e-3) / 1e9},
         "mean_iterations": float(it.mean()), "mean_pivots": float(piv.mean()), "mean_support": float(k.mean()),
     }
@@ -452,7 +483,7 @@ def main():
             "shared_sigma": {"value": world * N / (ms_shared * 1e-3), "unit": UNIT, "ms_per_step": ms_shared,
                              "what": "same step with ONE shared sigma[L] (sigma_pixel_stride = 0), device-resident"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
-            "cpu_baseline": cpu_baseline, "parity_sample": parity, "extras": extras,
+            "cpu_baseline": cpu_baseline, "parity_sample": parity, "histograms": histograms, "extras": extras,
         }
         print(json.dumps(line))
     if world > 1:

@@ -1,4 +1,4 @@
-// fp32_probe.cu -- FP32 FMA-pipe probe for the roofline denominator: a bench-side helper built into its own
+// fp32_probe.cu -- FP32 FMA-pipe probe for the roofline denominator: a bench-side helper (beside bench.py) built into its own
 // library (libfp32probe.so), NOT part of liblinmin.so or of include/linmin.h.
 // MEASURED_PEAKS.json carries HBM and bf16 tensor figures only; the path here is bound by plain FP32
 // arithmetic, so bench.py measures what the FMA pipe sustains: every thread runs

@@ -11,7 +11,6 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblinmin.so")
-PROBE_LIB = os.path.join(HERE, "libfp32probe.so")     # bench-side helper (roofline denominator), not the product
 # source -> extra flags of its translation unit
 SOURCES = {"linmin_api.cu": [], "finish_sweep.cu": [], "thresholds_static.cu": []}
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -19,7 +18,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
 
 
 def _deps():
-    out = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h")) and f != "fp32_probe.cu"]
+    out = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h"))]
     out.append(os.path.join(os.path.dirname(HERE), "include", "linmin.h"))
     return out
 
@@ -52,19 +51,5 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_probe(force: bool = False) -> str:
-    """libfp32probe.so: the FP32 FMA-pipe micro-benchmark bench.py reports next to the derived peak."""
-    src = os.path.join(CSRC, "fp32_probe.cu")
-    if not force and os.path.exists(PROBE_LIB) and os.path.getmtime(PROBE_LIB) >= os.path.getmtime(src):
-        return PROBE_LIB
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    tmp = PROBE_LIB + f".tmp{os.getpid()}"
-    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-                           "-Xcompiler", "-fPIC", "-shared", "-o", tmp, src, "-lcudart"])
-    os.replace(tmp, PROBE_LIB)
-    return PROBE_LIB
-
-
 if __name__ == "__main__":
     print(build_library(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
-    print(build_probe(force="--force" in sys.argv))

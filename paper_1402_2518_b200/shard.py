@@ -28,6 +28,27 @@ def cube_block(rank: int, cubes_per_rank: int) -> Tuple[int, int]:
     return rank * cubes_per_rank, (rank + 1) * cubes_per_rank
 
 
+def launch_plan(gpus: int, environ, visible_devices: int, argv, python: str, port: int):
+    """How `bench.py --gpus N` starts its ranks.  Returns ("inline", None) when this process is a rank already
+    (WORLD_SIZE set by torchrun) or one GPU is asked for, else ("spawn", cmd): the torchrun command line that starts
+    one rank per GPU on this node with the same arguments (rendezvous on 127.0.0.1: the container's hostname may not
+    resolve).  Asking for more GPUs than the node shows is an error, never a silent one-rank run."""
+    if gpus < 1:
+        raise ValueError("--gpus must be >= 1")
+    if "WORLD_SIZE" in environ:
+        world = int(environ["WORLD_SIZE"])
+        if world != gpus:
+            raise ValueError(f"--gpus {gpus} but the launcher started WORLD_SIZE={world} ranks")
+        return "inline", None
+    if gpus == 1:
+        return "inline", None
+    if visible_devices < gpus:
+        raise ValueError(f"--gpus {gpus} but only {visible_devices} CUDA device(s) are visible on this node")
+    cmd = [python, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port)] + list(argv)
+    return "spawn", cmd
+
+
 def max_over_ranks(value: float, device=None) -> float:
     """Maximum of a per-rank scalar (step time) over the process group; identity without a group."""
     import torch

@@ -10,7 +10,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_1402_2518_b200.shard import cube_block, pixel_block
+from paper_1402_2518_b200.shard import cube_block, launch_plan, pixel_block
 
 
 def test_pixel_block_partitions():
@@ -25,6 +25,24 @@ def test_pixel_block_partitions():
     with pytest.raises(ValueError):
         pixel_block(10, 2, 2)
     assert cube_block(3, 128) == (384, 512)
+
+
+def test_bench_launch_plan():
+    """`python bench.py --gpus N` must end up with N ranks: inline under torchrun or for one GPU, a torchrun command
+    line otherwise, and a loud error when the node has fewer devices (never a silent one-rank run labelled N)."""
+    argv = ["bench.py", "--gpus", "4", "--steps", "2"]
+    assert launch_plan(1, {}, 0, argv, "python", 29500) == ("inline", None)
+    assert launch_plan(4, {"WORLD_SIZE": "4", "RANK": "1"}, 8, argv, "python", 29500) == ("inline", None)
+    kind, cmd = launch_plan(4, {}, 8, argv, "py", 29511)
+    assert kind == "spawn" and cmd[:3] == ["py", "-m", "torch.distributed.run"] and cmd[-5:] == argv
+    assert "--nproc-per-node=4" in cmd and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29511"
+    with pytest.raises(ValueError, match="only 1 CUDA device"):
+        launch_plan(8, {}, 1, argv, "python", 29500)
+    with pytest.raises(ValueError, match="WORLD_SIZE=2"):
+        launch_plan(4, {"WORLD_SIZE": "2"}, 8, argv, "python", 29500)
+    with pytest.raises(ValueError):
+        launch_plan(0, {}, 8, argv, "python", 29500)
 
 
 def _free_port():
