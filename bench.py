@@ -223,6 +223,18 @@ def run_extras(linmin, torch, dev, A4, Yd, Sd):
         ms = time_calls(torch, lambda: linmin.unmix_lib(lib, Y1, None if "cov" in kw else S1))
         out["options"][label] = {"N": n, "ms": ms, "spectra_per_s": n / (ms * 1e-3)}
         lib.destroy()
+    # the one-shot form repeats the once-per-library precompute in every call (include/linmin.h): what that costs on one
+    # OMEGA-like cube, unweighted and with the full covariance (Cholesky factor + inverse of an L x L matrix per call)
+    n1 = min(CUBE, Yd.shape[0])
+    Yc, Sc = Yd[:n1], Sd[:n1]
+    out["one_shot"] = {"N": n1}
+    for label, kw in (("unweighted", dict()), ("full covariance", dict(cov=C.contiguous()))):
+        lib = linmin.library_create(Ad, **kw)
+        sg = None if kw else Sc
+        ms_h = time_calls(torch, lambda: linmin.unmix_lib(lib, Yc, sg))
+        ms_o = time_calls(torch, lambda: linmin.unmix(Ad, Yc, sg, **kw))
+        out["one_shot"][label] = {"handle_ms": ms_h, "one_shot_ms": ms_o, "precompute_ms": ms_o - ms_h}
+        lib.destroy()
     return out
 
 
